@@ -1,0 +1,169 @@
+/* dyplan.h -- C ABI of the B200-native physical-plan compiler hot path ("dyplan").
+ *
+ * What it computes (citations: PAPER.md:N = line N of the paper text; BJ = BASELINE.json):
+ *   A request is a materialised workflow DAG whose LLM nodes each choose one complete implementation
+ *   (model x verification policy x backend = one "option") -- PAPER.md:114-121 Eq.(1), Eq.(3) l.1.
+ *   For every plan pi (one option per node) and every backend-pressure level l the library evaluates
+ *     C(pi)   = prod_n (1 - v_n (1 - a_{n,k_n}))                    impact-weighted error f = v*(1-q),
+ *                                                                   PAPER.md:174-176; product form BJ:north_star
+ *     T_l(pi) = longest path of the pressure-scaled durations      PAPER.md:180, Eq.(3)
+ *               d_l(n,k) = floor(tau_{n,k} * mult[l][backend_{n,k}] / 1000)
+ *     D_b(pi) = sum_n demand_{n,k_n} [backend_{n,k_n} = b]          PAPER.md:203-211 (demand annotations)
+ *   and keeps, per (request, level), the best plan with T_l <= SLO and D_b <= cap_b under the fixed order
+ *   (C descending, T ascending, canonical plan index ascending) -- the pressure-specialised variants of
+ *   Algorithm 1, found by exhaustive enumeration instead of K ILP solves.
+ *   dyplan_replan does the same over the undispatched nodes only (App. D Eq.(7));
+ *   dyplan_select re-scores the stored variants under one live pressure vector and returns the variant
+ *   index per request without re-solving.
+ *
+ * Memory: the dyplan_batch / dyplan_bundle structs live in HOST memory.  In the plain calls every pointer
+ *   field is a DEVICE pointer on the ctx's device; in the *_host calls every pointer field is a HOST pointer
+ *   (the library stages the copies itself, on `stream`, and returns after the results are in the host buffers).
+ *   The caller owns every buffer and keeps it alive until the stream work completes.  The library allocates only
+ *   its own scratch inside dyplan_ctx (grown on demand; growing calls cudaMalloc, nothing else synchronises).
+ * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Plain calls are
+ *   asynchronous on it.  A ctx is not thread-safe; separate ctxs are independent.
+ * Errors: every call returns 0 or a negative DYPLAN_ERR_* code; nothing throws, aborts or prints.  Problems
+ *   only a device can see (malformed DAG, out-of-range table entries, NaN, overflow, plan space too large,
+ *   dispatched set not predecessor-closed) are reported per request in dyplan_bundle.status; the other requests
+ *   of the batch still compile.
+ * There is no CPU fallback: without a CUDA device dyplan_create fails with DYPLAN_ERR_CUDA.
+ */
+#ifndef DYPLAN_H_
+#define DYPLAN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* every entry point below is exported from libdyplan.so (the library is built with hidden default visibility) */
+#if defined(__GNUC__)
+#define DYPLAN_API __attribute__((visibility("default")))
+#else
+#define DYPLAN_API
+#endif
+
+#define DYPLAN_MAX_NODES 16   /* nodes per request                      */
+#define DYPLAN_MAX_OPTS 16    /* options per node                       */
+#define DYPLAN_MAX_BACKENDS 8
+#define DYPLAN_MAX_MODELS 8
+#define DYPLAN_MAX_LEVELS 8   /* pressure levels per compile call       */
+#define DYPLAN_MAX_PLANS_LOG2 40 /* enumerated plans per request <= 2^40 */
+
+/* return codes */
+#define DYPLAN_OK 0
+#define DYPLAN_ERR_NULL (-1)   /* a required pointer is NULL                               */
+#define DYPLAN_ERR_LIMIT (-2)  /* R, B, M, L, NN or KK outside the limits above / negative  */
+#define DYPLAN_ERR_CUDA (-3)   /* a CUDA runtime call failed; see dyplan_last_cuda_error()  */
+#define DYPLAN_ERR_ARG (-4)    /* unknown flag bits, inconsistent sizes                     */
+
+/* per-(request, level) status in dyplan_bundle.status */
+#define DYPLAN_ST_OK 0         /* a feasible best plan was found                            */
+#define DYPLAN_ST_INFEASIBLE 1 /* no plan meets SLO and caps (sentinel outputs)             */
+#define DYPLAN_ST_INVALID 2    /* malformed request (sentinel outputs)                      */
+#define DYPLAN_ST_TOO_LARGE 3  /* more than 2^40 plans to enumerate (sentinel outputs)      */
+
+/* dyplan_replan flags (reading Q10: both readings of App. D are offered) */
+#define DYPLAN_FIXED_IN_PLACE 0u /* dispatched nodes keep their latency, factor and demand (BJ:configs[3])          */
+#define DYPLAN_RESIDUAL 1u       /* dispatched nodes contribute d=0, factor 1, demand 0 ("residual makespan T_t starts
+                                    from zero on G_t and spans only undispatched work")               */
+
+typedef struct dyplan_ctx dyplan_ctx;
+
+/* A batch of R requests (or replan queries).  The nodes of a request are listed in a topological order
+ * (a finite DAG; branches resolved and loops unrolled before submission).  A tool node is a node with
+ * one option (fixed duration, no choice).  NN = node_off[R], KK = opt_off[NN]. */
+typedef struct {
+  int32_t R;                 /* requests, >= 0                                                                */
+  int32_t B;                 /* backends, 1..8                                                                */
+  int32_t M;                 /* models, 1..8 (annotations only)                                               */
+  int32_t NN;                /* total nodes   (= node_off[R]); bounds every per-node array                    */
+  int32_t KK;                /* total options (= opt_off[NN]); bounds every per-option array                  */
+  const int32_t* node_off;   /* [R+1]  prefix offsets into the per-node arrays; 0 <= N_r <= 16                */
+  const int32_t* opt_off;    /* [NN+1] prefix offsets into the per-option arrays; 1 <= K_n <= 16              */
+  const uint32_t* pred_mask; /* [NN]   bit p set => local node p precedes node n; requires p < n             */
+  const float* vuln;         /* [NN]   vulnerability v_n in [0,1]; NaN is invalid, not zero   */
+  const int32_t* lat_us;     /* [KK]   nominal duration tau_{n,k} >= 0, microseconds                         */
+  const float* acc;          /* [KK]   a_{n,k} in [0,1], quality of the complete model+verifier pair         */
+  const int32_t* demand;     /* [KK]   token demand >= 0                                                     */
+  const uint8_t* backend;    /* [KK]   < B                                                                   */
+  const uint8_t* model;      /* [KK]   < M                                                                   */
+  const int32_t* slo_us;     /* [R]    latency SLO >= 0, inclusive                                           */
+  const int32_t* cap;        /* [R*B]  per-backend demand cap >= 0, inclusive; NULL = no caps                */
+} dyplan_batch;
+
+/* Result: one record per (request, level) at index rec = r*L + l.  Sentinels when status != OK:
+ * plan_idx = UINT64_MAX, choice = 0xFF.., corr = -1, corr64 = -1, lat = INT32_MAX, dem = 0, dom_model = 0xFF. */
+typedef struct {
+  uint64_t* plan_idx; /* [R*L]    canonical mixed-radix index sum_n k_n prod_{t<n} K_t (node 0 least significant)  */
+  uint8_t* choice;    /* [R*L*16] chosen option per node, 0xFF padding                                        */
+  float* corr;        /* [R*L]    C(pi) as the scorer computed it (fp32)                                       */
+  double* corr64;     /* [R*L]    C(pi) of the chosen plan re-evaluated in fp64, node order; may be NULL       */
+  int32_t* lat;       /* [R*L]    T_l(pi), microseconds                                                        */
+  int32_t* dem;       /* [R*L*B]  per-backend demand D_b(pi)                                                   */
+  uint8_t* dom_model; /* [R*L]    model with the largest planned demand, ties -> lowest id     */
+  uint8_t* status;    /* [R*L]    DYPLAN_ST_*                                                                 */
+} dyplan_bundle;
+
+/* Create / destroy a context on CUDA device `device_ordinal`.  Fails (DYPLAN_ERR_CUDA) without a device. */
+DYPLAN_API int dyplan_create(dyplan_ctx** out, int device_ordinal);
+DYPLAN_API int dyplan_destroy(dyplan_ctx* ctx);
+
+/* Algorithm 1 l.10-15 by exhaustive enumeration: best plan per (request, level).
+ * mult_pm: [L*B] per-mille latency multipliers >= 0 per (level, backend) -- device pointer (host in *_host). */
+DYPLAN_API int dyplan_compile(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
+                   void* stream);
+
+/* App. D Eq.(7): re-optimise the undispatched nodes of each query, committed bindings fixed
+ * ("the merge rejects overlap instead of replacing a committed binding": choice[n] == fixed_choice[n]
+ * on dispatched nodes).  dispatched_mask [R]: bit n set => local node n already dispatched; must be predecessor-
+ * closed, else status INVALID.  fixed_choice [NN]: read where dispatched.  live_mult_pm [R*B]: one
+ * live multiplier vector per query.  out holds one record per query (L = 1).  All nodes dispatched => exactly one
+ * plan is scored. */
+DYPLAN_API int dyplan_replan(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask, const uint8_t* fixed_choice,
+                  const int32_t* live_mult_pm, uint32_t flags, dyplan_bundle* out, void* stream);
+
+/* Section 5.1 as a stateless re-scoring: for each request re-score the L stored variants of
+ * `bundle` (uses bundle->choice and bundle->status only) under ONE live multiplier vector live_mult_pm [B] and return
+ * variant[r] in [0,L), ordered by (SLO-feasible under the live vector first; then C desc, T' asc, l asc; if no stored
+ * variant is feasible: T' asc, C desc, l asc); -1 if the bundle holds no plan for the request.  `rescored` (optional,
+ * one record per request, L = 1) receives the picked variant re-scored; its status is OK or INFEASIBLE (picked but
+ * over the SLO) or the stored error. */
+DYPLAN_API int dyplan_select(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L,
+                  const int32_t* live_mult_pm, int32_t* variant, dyplan_bundle* rescored, void* stream);
+
+/* Same three calls with HOST pointers everywhere (batch fields, multipliers, masks, outputs).  The library copies
+ * inputs to the device, runs the same kernels and copies the results back, all on `stream`, and returns after a
+ * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied. */
+DYPLAN_API int dyplan_compile_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
+                        void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+DYPLAN_API int dyplan_replan_host(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask,
+                       const uint8_t* fixed_choice, const int32_t* live_mult_pm, uint32_t flags, dyplan_bundle* out,
+                       void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+DYPLAN_API int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L,
+                       const int32_t* live_mult_pm, int32_t* variant, dyplan_bundle* rescored, void* stream,
+                       uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
+/* Introspection for the bench and the tests (no device synchronisation unless stated). */
+typedef struct {
+  uint64_t plans;       /* plans enumerated by the last compile/replan (sum over valid requests)                 */
+  uint64_t evals;       /* (plan, level) evaluations = sum_r plans_r * L                                          */
+  uint64_t work_items;  /* (request, plan-range) work items the scorer processed                                  */
+  uint64_t slow_steps;  /* inner blocks that took the exact (slow) path                                           */
+  int32_t launches;     /* kernels launched by the last call                                                      */
+  int32_t sm_count;     /* SMs of the device                                                                      */
+  float score_ms;       /* device time of the scoring kernel of the last call (CUDA events on `stream`)           */
+} dyplan_stats;
+/* Synchronises `stream` of the last call, then fills *out. */
+DYPLAN_API int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out);
+
+DYPLAN_API const char* dyplan_strerror(int code);
+DYPLAN_API const char* dyplan_last_cuda_error(const dyplan_ctx* ctx); /* "" if none */
+DYPLAN_API int dyplan_version(void);                            /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DYPLAN_H_ */

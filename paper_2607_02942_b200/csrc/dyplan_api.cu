@@ -1,0 +1,440 @@
+// dyplan_api.cu -- the C ABI of include/dyplan.h: argument checks, scratch management, kernel sequencing.
+// No arithmetic of the method lives here; every step of the path runs in the kernels.
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "dyplan_internal.cuh"
+
+namespace dyplan {
+cudaError_t launch_score_l1(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l2(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l3(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l4(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l5(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l6(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l7(const CallArgs&, int, int, cudaStream_t);
+cudaError_t launch_score_l8(const CallArgs&, int, int, cudaStream_t);
+int score_occupancy_l1(int);
+int score_occupancy_l2(int);
+int score_occupancy_l3(int);
+int score_occupancy_l4(int);
+int score_occupancy_l5(int);
+int score_occupancy_l6(int);
+int score_occupancy_l7(int);
+int score_occupancy_l8(int);
+static const score_launcher_t kLaunch[8] = {launch_score_l1, launch_score_l2, launch_score_l3, launch_score_l4,
+                                            launch_score_l5, launch_score_l6, launch_score_l7, launch_score_l8};
+typedef int (*occ_fn_t)(int);
+static const occ_fn_t kOcc[8] = {score_occupancy_l1, score_occupancy_l2, score_occupancy_l3, score_occupancy_l4,
+                                 score_occupancy_l5, score_occupancy_l6, score_occupancy_l7, score_occupancy_l8};
+}  // namespace dyplan
+
+using namespace dyplan;
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+};
+
+struct dyplan_ctx {
+  int device = 0;
+  int sm_count = 0;
+  cudaError_t last_err = cudaSuccess;
+  char errbuf[256] = {0};
+  // scratch
+  DevBuf blob, item_off, done, gthr, partial, state;
+  // staging for the *_host calls: one device arena, one pinned-or-not host side is the caller's
+  DevBuf arena;
+  // occupancy cache [L-1][nb index]
+  int occ[8][4];
+  // last call
+  cudaStream_t last_stream = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool have_events = false;
+  int last_launches = 0;
+  int last_L = 0;
+};
+
+static int fail_cuda(dyplan_ctx* c, cudaError_t e) {
+  c->last_err = e;
+  snprintf(c->errbuf, sizeof(c->errbuf), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return DYPLAN_ERR_CUDA;
+}
+#define CK(call)                                        \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) return fail_cuda(ctx, e__); \
+  } while (0)
+
+static int ensure(dyplan_ctx* ctx, DevBuf& b, size_t bytes) {
+  if (bytes <= b.cap) return DYPLAN_OK;
+  if (b.p) CK(cudaFree(b.p));
+  b.p = nullptr; b.cap = 0;
+  size_t want = bytes + bytes / 4 + 256;
+  CK(cudaMalloc(&b.p, want));
+  b.cap = want;
+  return DYPLAN_OK;
+}
+
+static int nb_index(int nb_class) { return nb_class == 0 ? 0 : nb_class == 2 ? 1 : nb_class == 4 ? 2 : 3; }
+
+extern "C" {
+
+int dyplan_version(void) { return 100; }
+
+const char* dyplan_strerror(int code) {
+  switch (code) {
+    case DYPLAN_OK: return "ok";
+    case DYPLAN_ERR_NULL: return "a required pointer is NULL";
+    case DYPLAN_ERR_LIMIT: return "R, B, M, L, NN or KK outside the supported limits";
+    case DYPLAN_ERR_CUDA: return "a CUDA runtime call failed (see dyplan_last_cuda_error)";
+    case DYPLAN_ERR_ARG: return "invalid argument";
+    default: return "unknown error";
+  }
+}
+
+const char* dyplan_last_cuda_error(const dyplan_ctx* ctx) { return ctx ? ctx->errbuf : ""; }
+
+int dyplan_create(dyplan_ctx** out, int device_ordinal) {
+  if (!out) return DYPLAN_ERR_NULL;
+  *out = nullptr;
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || device_ordinal < 0 || device_ordinal >= n) return DYPLAN_ERR_CUDA;
+  dyplan_ctx* ctx = new (std::nothrow) dyplan_ctx();
+  if (!ctx) return DYPLAN_ERR_ARG;
+  ctx->device = device_ordinal;
+  if (cudaSetDevice(device_ordinal) != cudaSuccess ||
+      cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device_ordinal) != cudaSuccess ||
+      cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
+    delete ctx;
+    return DYPLAN_ERR_CUDA;
+  }
+  for (int i = 0; i < 8; i++) for (int j = 0; j < 4; j++) ctx->occ[i][j] = 0;
+  *out = ctx;
+  return DYPLAN_OK;
+}
+
+int dyplan_destroy(dyplan_ctx* ctx) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  cudaSetDevice(ctx->device);
+  DevBuf* bufs[] = {&ctx->blob, &ctx->item_off, &ctx->done, &ctx->gthr, &ctx->partial, &ctx->state, &ctx->arena};
+  for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
+  if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+  if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+  delete ctx;
+  return DYPLAN_OK;
+}
+
+}  // extern "C"
+
+static int check_batch(const dyplan_batch* in, bool need_arrays) {
+  if (!in) return DYPLAN_ERR_NULL;
+  if (in->R < 0 || in->B < 1 || in->B > DYPLAN_MAX_BACKENDS || in->M < 1 || in->M > DYPLAN_MAX_MODELS || in->NN < 0 ||
+      in->KK < 0 || in->R > (1 << 24))
+    return DYPLAN_ERR_LIMIT;
+  if (need_arrays && in->R > 0) {
+    if (!in->node_off || !in->opt_off || !in->slo_us) return DYPLAN_ERR_NULL;
+    if (in->NN > 0 && (!in->pred_mask || !in->vuln)) return DYPLAN_ERR_NULL;
+    if (in->KK > 0 && (!in->lat_us || !in->acc || !in->demand || !in->backend || !in->model)) return DYPLAN_ERR_NULL;
+  }
+  return DYPLAN_OK;
+}
+
+static int check_bundle(const dyplan_bundle* o) {
+  if (!o) return DYPLAN_ERR_NULL;
+  if (!o->plan_idx || !o->choice || !o->corr || !o->lat || !o->dem || !o->dom_model || !o->status) return DYPLAN_ERR_NULL;
+  return DYPLAN_OK;
+}
+
+// compile and replan share everything but two arguments
+static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult, const uint32_t* dispatched,
+                     const uint8_t* fixed_choice, uint32_t flags, bool is_replan, dyplan_bundle* out, cudaStream_t stream) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = check_batch(in, true);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  if (flags & ~DYPLAN_RESIDUAL) return DYPLAN_ERR_ARG;
+  ctx->last_launches = 0;
+  ctx->have_events = false;
+  ctx->last_stream = stream;
+  ctx->last_L = L;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!mult) return DYPLAN_ERR_NULL;
+  if (is_replan && (!dispatched || (in->NN > 0 && !fixed_choice))) return DYPLAN_ERR_NULL;
+  rc = check_bundle(out);
+  if (rc) return rc;
+  CK(cudaSetDevice(ctx->device));
+
+  const size_t R = (size_t)in->R;
+  const uint32_t max_items = (uint32_t)(R + 32768);
+  if ((rc = ensure(ctx, ctx->blob, R * blob_stride_words(L) * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->item_off, (R + 1) * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->done, R * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->gthr, R * L * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->partial, (size_t)max_items * L * sizeof(Partial)))) return rc;
+  if ((rc = ensure(ctx, ctx->state, sizeof(CallState)))) return rc;
+
+  CallArgs a;
+  memset(&a, 0, sizeof(a));
+  a.in = *in; a.out = *out; a.L = L; a.mult = mult; a.dispatched = dispatched; a.fixed_choice = fixed_choice;
+  a.flags = flags; a.is_replan = is_replan ? 1 : 0;
+  a.blob = (uint32_t*)ctx->blob.p; a.item_off = (uint32_t*)ctx->item_off.p; a.done = (uint32_t*)ctx->done.p;
+  a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
+  a.max_items = max_items;
+
+  const int nbc = nb_class_of(in->B, in->cap != nullptr);
+  int& occ = ctx->occ[L - 1][nb_index(nbc)];
+  if (occ <= 0) {
+    occ = kOcc[L - 1](nbc);
+    if (occ <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
+  }
+  const int grid = ctx->sm_count * occ;   // persistent: every block resident, work pulled from a device counter
+
+  CK(launch_stage(a, stream));
+  CK(launch_plan(a, stream));
+  CK(cudaEventRecord(ctx->ev0, stream));
+  CK(kLaunch[L - 1](a, nbc, grid, stream));
+  CK(cudaEventRecord(ctx->ev1, stream));
+  ctx->have_events = true;
+  ctx->last_launches = 3;
+  return DYPLAN_OK;
+}
+
+extern "C" {
+
+int dyplan_compile(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out, void* stream) {
+  return run_solve(ctx, in, L, mult_pm, nullptr, nullptr, 0, false, out, (cudaStream_t)stream);
+}
+
+int dyplan_replan(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask, const uint8_t* fixed_choice,
+                  const int32_t* live_mult_pm, uint32_t flags, dyplan_bundle* out, void* stream) {
+  return run_solve(ctx, in, 1, live_mult_pm, dispatched_mask, fixed_choice, flags, true, out, (cudaStream_t)stream);
+}
+
+int dyplan_select(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L, const int32_t* live_mult_pm,
+                  int32_t* variant, dyplan_bundle* rescored, void* stream) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = check_batch(in, true);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  ctx->last_launches = 0;
+  ctx->have_events = false;
+  ctx->last_stream = (cudaStream_t)stream;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!bundle || !bundle->choice || !bundle->status || !live_mult_pm || !variant) return DYPLAN_ERR_NULL;
+  if (rescored && (rc = check_bundle(rescored))) return rc;
+  CK(cudaSetDevice(ctx->device));
+  SelectArgs a;
+  memset(&a, 0, sizeof(a));
+  a.in = *in; a.choice = bundle->choice; a.status = bundle->status; a.L = L; a.live = live_mult_pm; a.variant = variant;
+  if (rescored) { a.rescored = *rescored; a.has_rescored = 1; }
+  CK(launch_select(a, (cudaStream_t)stream));
+  ctx->last_launches = 1;
+  return DYPLAN_OK;
+}
+
+int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
+  if (!ctx || !out) return DYPLAN_ERR_NULL;
+  memset(out, 0, sizeof(*out));
+  out->sm_count = ctx->sm_count;
+  out->launches = ctx->last_launches;
+  CK(cudaSetDevice(ctx->device));
+  CK(cudaStreamSynchronize(ctx->last_stream));
+  if (ctx->have_events && ctx->state.p) {
+    CallState st;
+    CK(cudaMemcpy(&st, ctx->state.p, sizeof(st), cudaMemcpyDeviceToHost));
+    out->plans = st.total_plans;
+    out->evals = st.total_plans * (uint64_t)ctx->last_L;
+    out->work_items = st.total_items;
+    out->slow_steps = st.slow_steps;
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    out->score_ms = ms;
+  }
+  return DYPLAN_OK;
+}
+
+}  // extern "C"
+
+// ---- *_host calls: stage the copies, run the same kernels, copy back ---------------------------------------------
+namespace {
+
+struct Arena {
+  char* base;
+  size_t off;
+  template <typename T>
+  T* take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = (T*)(base + off);
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+struct HostPlan {   // sizes of everything a call moves
+  size_t R, NN, KK, B, L, nrec;
+};
+
+size_t arena_bytes(const HostPlan& p) {
+  // generous: every array rounded to 256 B
+  size_t n = 0;
+  auto add = [&](size_t bytes) { n += ((bytes + 255) & ~(size_t)255) + 256; };
+  add((p.R + 1) * 4); add((p.NN + 1) * 4); add(p.NN * 4); add(p.NN * 4);
+  add(p.KK * 4); add(p.KK * 4); add(p.KK * 4); add(p.KK); add(p.KK);
+  add(p.R * 4); add(p.R * p.B * 4);
+  add(p.L * p.B * 4 + p.R * p.B * 4); add(p.R * 4); add(p.NN);
+  // outputs (two bundles at most: stored + rescored) + variant
+  for (int i = 0; i < 2; i++) {
+    add(p.nrec * 8); add(p.nrec * 16); add(p.nrec * 4); add(p.nrec * 8); add(p.nrec * 4); add(p.nrec * p.B * 4); add(p.nrec); add(p.nrec);
+  }
+  add(p.R * 4);
+  return n;
+}
+
+}  // namespace
+
+#define H2D(dst, src, n, T)                                                                            \
+  do {                                                                                                 \
+    dst = ar.take<T>(n);                                                                               \
+    if ((n) > 0) { CK(cudaMemcpyAsync((void*)dst, src, (size_t)(n) * sizeof(T), cudaMemcpyHostToDevice, s)); h2d += (size_t)(n) * sizeof(T); } \
+  } while (0)
+
+static int batch_to_device(dyplan_ctx* ctx, const dyplan_batch* in, Arena& ar, dyplan_batch* d, cudaStream_t s, uint64_t& h2d) {
+  *d = *in;
+  int32_t *node_off, *opt_off, *lat, *dem, *slo, *cap = nullptr;
+  uint32_t* pm; float *vuln, *acc; uint8_t *be, *mo;
+  H2D(node_off, in->node_off, (size_t)in->R + 1, int32_t);
+  H2D(opt_off, in->opt_off, (size_t)in->NN + 1, int32_t);
+  H2D(pm, in->pred_mask, (size_t)in->NN, uint32_t);
+  H2D(vuln, in->vuln, (size_t)in->NN, float);
+  H2D(lat, in->lat_us, (size_t)in->KK, int32_t);
+  H2D(acc, in->acc, (size_t)in->KK, float);
+  H2D(dem, in->demand, (size_t)in->KK, int32_t);
+  H2D(be, in->backend, (size_t)in->KK, uint8_t);
+  H2D(mo, in->model, (size_t)in->KK, uint8_t);
+  H2D(slo, in->slo_us, (size_t)in->R, int32_t);
+  if (in->cap) H2D(cap, in->cap, (size_t)in->R * in->B, int32_t);
+  d->node_off = node_off; d->opt_off = opt_off; d->pred_mask = pm; d->vuln = vuln; d->lat_us = lat; d->acc = acc;
+  d->demand = dem; d->backend = be; d->model = mo; d->slo_us = slo; d->cap = cap;
+  return DYPLAN_OK;
+}
+
+static void bundle_alloc(Arena& ar, size_t nrec, size_t B, bool want64, dyplan_bundle* d) {
+  d->plan_idx = ar.take<uint64_t>(nrec); d->choice = ar.take<uint8_t>(nrec * 16); d->corr = ar.take<float>(nrec);
+  d->corr64 = want64 ? ar.take<double>(nrec) : nullptr; d->lat = ar.take<int32_t>(nrec); d->dem = ar.take<int32_t>(nrec * B);
+  d->dom_model = ar.take<uint8_t>(nrec); d->status = ar.take<uint8_t>(nrec);
+}
+
+#define D2H(dst, src, n, T)                                                                              \
+  do {                                                                                                   \
+    if ((n) > 0 && (dst)) { CK(cudaMemcpyAsync((void*)(dst), src, (size_t)(n) * sizeof(T), cudaMemcpyDeviceToHost, s)); d2h += (size_t)(n) * sizeof(T); } \
+  } while (0)
+
+static int bundle_to_host(dyplan_ctx* ctx, const dyplan_bundle* d, dyplan_bundle* h, size_t nrec, size_t B, cudaStream_t s, uint64_t& d2h) {
+  D2H(h->plan_idx, d->plan_idx, nrec, uint64_t);
+  D2H(h->choice, d->choice, nrec * 16, uint8_t);
+  D2H(h->corr, d->corr, nrec, float);
+  if (d->corr64) D2H(h->corr64, d->corr64, nrec, double);
+  D2H(h->lat, d->lat, nrec, int32_t);
+  D2H(h->dem, d->dem, nrec * B, int32_t);
+  D2H(h->dom_model, d->dom_model, nrec, uint8_t);
+  D2H(h->status, d->status, nrec, uint8_t);
+  return DYPLAN_OK;
+}
+
+static int host_sizes_ok(const dyplan_batch* in) {
+  int rc = check_batch(in, true);
+  if (rc) return rc;
+  if (in->R > 0 && (in->node_off[in->R] != in->NN)) return DYPLAN_ERR_ARG;
+  if (in->R > 0 && in->NN > 0 && in->opt_off[in->NN] != in->KK) return DYPLAN_ERR_ARG;
+  return DYPLAN_OK;
+}
+
+static int solve_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult, const uint32_t* dispatched,
+                      const uint8_t* fixed_choice, uint32_t flags, bool is_replan, dyplan_bundle* out, void* stream,
+                      uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = host_sizes_ok(in);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  uint64_t h2d = 0, d2h = 0;
+  if (h2d_bytes) *h2d_bytes = 0;
+  if (d2h_bytes) *d2h_bytes = 0;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!mult || (is_replan && (!dispatched || (in->NN > 0 && !fixed_choice)))) return DYPLAN_ERR_NULL;
+  if ((rc = check_bundle(out))) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  HostPlan hp{(size_t)in->R, (size_t)in->NN, (size_t)in->KK, (size_t)in->B, (size_t)L, (size_t)in->R * L};
+  if ((rc = ensure(ctx, ctx->arena, arena_bytes(hp)))) return rc;
+  Arena ar{(char*)ctx->arena.p, 0};
+  dyplan_batch d;
+  if ((rc = batch_to_device(ctx, in, ar, &d, s, h2d))) return rc;
+  int32_t* dmult; uint32_t* ddisp = nullptr; uint8_t* dfix = nullptr;
+  H2D(dmult, mult, is_replan ? (size_t)in->R * in->B : (size_t)L * in->B, int32_t);
+  if (is_replan) { H2D(ddisp, dispatched, (size_t)in->R, uint32_t); H2D(dfix, fixed_choice, (size_t)in->NN, uint8_t); }
+  dyplan_bundle dout;
+  bundle_alloc(ar, hp.nrec, hp.B, out->corr64 != nullptr, &dout);
+  if ((rc = run_solve(ctx, &d, L, dmult, ddisp, dfix, flags, is_replan, &dout, s))) return rc;
+  if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h))) return rc;
+  CK(cudaStreamSynchronize(s));
+  if (h2d_bytes) *h2d_bytes = h2d;
+  if (d2h_bytes) *d2h_bytes = d2h;
+  return DYPLAN_OK;
+}
+
+extern "C" {
+
+int dyplan_compile_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
+                        void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  return solve_host(ctx, in, L, mult_pm, nullptr, nullptr, 0, false, out, stream, h2d_bytes, d2h_bytes);
+}
+
+int dyplan_replan_host(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask, const uint8_t* fixed_choice,
+                       const int32_t* live_mult_pm, uint32_t flags, dyplan_bundle* out, void* stream, uint64_t* h2d_bytes,
+                       uint64_t* d2h_bytes) {
+  if (flags & ~DYPLAN_RESIDUAL) return DYPLAN_ERR_ARG;
+  return solve_host(ctx, in, 1, live_mult_pm, dispatched_mask, fixed_choice, flags, true, out, stream, h2d_bytes, d2h_bytes);
+}
+
+int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L, const int32_t* live_mult_pm,
+                       int32_t* variant, dyplan_bundle* rescored, void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = host_sizes_ok(in);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  uint64_t h2d = 0, d2h = 0;
+  if (h2d_bytes) *h2d_bytes = 0;
+  if (d2h_bytes) *d2h_bytes = 0;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!bundle || !bundle->choice || !bundle->status || !live_mult_pm || !variant) return DYPLAN_ERR_NULL;
+  if (rescored && (rc = check_bundle(rescored))) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  HostPlan hp{(size_t)in->R, (size_t)in->NN, (size_t)in->KK, (size_t)in->B, (size_t)L, (size_t)in->R * L};
+  if ((rc = ensure(ctx, ctx->arena, arena_bytes(hp)))) return rc;
+  Arena ar{(char*)ctx->arena.p, 0};
+  dyplan_batch d;
+  if ((rc = batch_to_device(ctx, in, ar, &d, s, h2d))) return rc;
+  int32_t* dlive; uint8_t *dch, *dst;
+  H2D(dlive, live_mult_pm, (size_t)in->B, int32_t);
+  H2D(dch, bundle->choice, hp.nrec * 16, uint8_t);
+  H2D(dst, bundle->status, hp.nrec, uint8_t);
+  dyplan_bundle dbundle;
+  memset(&dbundle, 0, sizeof(dbundle));
+  dbundle.choice = dch; dbundle.status = dst;
+  int32_t* dvar = ar.take<int32_t>(hp.R);
+  dyplan_bundle dres;
+  if (rescored) bundle_alloc(ar, hp.R, hp.B, rescored->corr64 != nullptr, &dres);
+  if ((rc = dyplan_select(ctx, &d, &dbundle, L, dlive, dvar, rescored ? &dres : nullptr, stream))) return rc;
+  D2H(variant, dvar, hp.R, int32_t);
+  if (rescored && (rc = bundle_to_host(ctx, &dres, rescored, hp.R, hp.B, s, d2h))) return rc;
+  CK(cudaStreamSynchronize(s));
+  if (h2d_bytes) *h2d_bytes = h2d;
+  if (d2h_bytes) *d2h_bytes = d2h;
+  return DYPLAN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,107 @@
+// dyplan_internal.cuh -- structures shared by the kernels of libdyplan (product side only; the oracle
+// shares nothing with this directory).  See DESIGN.md sections 4-6 for the layout and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dyplan.h"
+
+namespace dyplan {
+
+constexpr int kBlock = 128;          // threads per scoring block
+constexpr int kHdrWords = 120;       // ReqHdr size in 4-byte words (multiple of 4 -> 16-byte aligned tables)
+constexpr int kMaxSlots = 16 * 16 + 4;  // option slots of one request incl. dummies, padded to 4
+constexpr int kDem0bWords = 16 * 8;  // per-backend demand of the inner node's options [k0][b]
+constexpr int kMaxBlobWords = kHdrWords + kDem0bWords + kMaxSlots * (DYPLAN_MAX_LEVELS + 3);
+// Every request owns a fixed-size blob (header, dem0b, lat[slot][L], f[slot], dem[slot], be[slot]); only the used
+// part is ever written or read, so the stride costs address space, not traffic.
+__host__ __device__ inline size_t blob_stride_words(int L) { return (size_t)kHdrWords + kDem0bWords + (size_t)kMaxSlots * (size_t)(L + 3); }
+constexpr uint64_t kNoIdx = ~0ull;
+
+// Per-request staged problem in "internal" node order.  Internal node 0 is the innermost
+// enumeration digit, node 1 the middle digit, nodes >= 2 the outer digits.  deps(i) only holds nodes j > i, so
+// the slack recurrence  u[i] = min(SLO, min_{j in deps(i)} u[j]) - d[i][k_i]  can be evaluated from the
+// outermost node inwards; the longest path is  T = SLO - min_i u[i]  (Eq.(3), in slack form).
+struct ReqHdr {
+  int32_t status;        // DYPLAN_ST_OK, _INVALID or _TOO_LARGE (input problems only)
+  int32_t n_int;         // internal nodes N' >= 3 (dummy nodes appended when N < 3)
+  int32_t n_orig;        // original nodes N
+  int32_t orient;        // 0: internal i = original i, deps = successors; 1: internal i = original N-1-i, deps = predecessors
+  int32_t K0, K1;        // real radices of internal nodes 0 and 1
+  int32_t K0p;           // inner radix class: K0 padded up to one of {2,4,6,8,12,16}
+  int32_t slo;
+  int32_t nslots_pad;    // option slots in the tables (multiple of 4)
+  int32_t n0;            // first original node (node_off[r])
+  int32_t conn01;        // 1 if internal node 1 is in deps(0)
+  uint32_t skip_mask;    // original nodes that contribute nothing (RESIDUAL replan)
+  unsigned long long outer_total;  // prod_{i>=2} K'_i : number of outer indices
+  unsigned long long base_idx;     // canonical-index contribution of the pinned (dispatched) nodes
+  int32_t cap[8];        // per-backend caps (INT32_MAX when absent)
+  int32_t Kp[16];        // enumerated radix per internal node (1 for pinned / dummy nodes)
+  uint32_t deps[16];     // dependency mask per internal node (internal indices, all > i)
+  int32_t optbase[16];   // first table slot of internal node i
+  int32_t fixk[16];      // unused (reserved)
+  unsigned long long stride[16];   // canonical stride of internal node i (0 for dummies / pinned nodes)
+};
+static_assert(sizeof(ReqHdr) == kHdrWords * 4, "ReqHdr layout");
+
+// partial best of one work item and one level
+struct __align__(16) Partial {
+  float C;
+  int32_t T;
+  unsigned long long idx;   // kNoIdx: none
+};
+
+// device-side counters / plan of one call
+struct CallState {
+  unsigned long long total_outer;   // sum over valid requests of outer_total
+  unsigned long long total_plans;   // sum over valid requests of enumerated plans
+  unsigned long long per_item_outer;
+  unsigned long long slow_steps;
+  uint32_t total_items;
+  uint32_t next_item;               // dynamic work counter
+  uint32_t mult_invalid;            // a multiplier was negative
+  uint32_t pad;
+};
+
+struct CallArgs {                   // passed by value to the kernels
+  dyplan_batch in;
+  dyplan_bundle out;
+  int32_t L;
+  const int32_t* mult;              // [L*B] (compile) or [R*B] (replan)
+  const uint32_t* dispatched;       // replan only
+  const uint8_t* fixed_choice;      // replan only
+  uint32_t flags;
+  int32_t is_replan;
+  // scratch
+  uint32_t* blob;                   // staged requests
+  uint32_t* item_off;               // [R+1]
+  uint32_t* done;                   // [R] ticket counters
+  float* gthr;                      // [R*L] published best C per (request, level)
+  Partial* partial;                 // [max_items * L]
+  CallState* st;
+  uint32_t max_items;
+};
+
+
+// launchers (defined in the .cu files)
+cudaError_t launch_stage(const CallArgs& a, cudaStream_t s);
+cudaError_t launch_plan(const CallArgs& a, cudaStream_t s);
+typedef cudaError_t (*score_launcher_t)(const CallArgs& a, int nb_class, int grid, cudaStream_t s);
+cudaError_t launch_score(const CallArgs& a, int grid, cudaStream_t s);
+int score_blocks_per_sm(int L, int nb_class);
+struct SelectArgs {
+  dyplan_batch in;
+  const uint8_t* choice;   // [R*L*16]
+  const uint8_t* status;   // [R*L]
+  int32_t L;
+  const int32_t* live;     // [B]
+  int32_t* variant;        // [R]
+  dyplan_bundle rescored;  // optional (pointers may be null)
+  int32_t has_rescored;
+};
+cudaError_t launch_select(const SelectArgs& a, cudaStream_t s);
+
+__host__ __device__ inline int nb_class_of(int B, bool has_caps) { return !has_caps ? 0 : (B <= 2 ? 2 : (B <= 4 ? 4 : 8)); }
+
+}  // namespace dyplan

@@ -1,0 +1,450 @@
+// dyplan_score.cuh -- K_score: enumerate + score + arg-best, one template per (L, NB).
+// Included by dyplan_score_l<L>.cu with DYPLAN_SCORE_L defined.  DESIGN.md section 6 explains the kernel.
+//
+// Per work item (a range of outer indices of one request) every thread walks its outer digits in odometer
+// order, keeps the slack DP of the outer nodes in local arrays, runs the middle digit (internal node 1) as a
+// loop and the inner digit (internal node 0) fully unrolled with its tables in registers:
+//
+//   per (plan, level):   t = a'_l - d0[k0][l]            slack of the only plan-dependent path (Eq.(3) in slack form)
+//                        y = C(plan) - bestC_l           sign says "not worse than the incumbent"
+//                        acc &= t | bits(y)              sign(acc) stays set while no candidate showed up
+//   per plan:            C = C1 * f0[k0]  (+ cap slack folded into the sign of C when caps are present)
+//
+// A prefix whose acc came out non-negative is re-walked by the exact slow path, which applies the full order
+// (C desc, T asc, canonical index asc) and updates the thread's incumbent.
+#pragma once
+#include "dyplan_internal.cuh"
+
+namespace dyplan {
+
+struct Best {
+  float C;
+  int32_t T;
+  unsigned long long idx;
+};
+
+__device__ __forceinline__ bool better(float C, int T, unsigned long long idx, const Best& b) {
+  if (idx == kNoIdx) return false;
+  if (b.idx == kNoIdx) return true;
+  if (C != b.C) return C > b.C;
+  if (T != b.T) return T < b.T;
+  return idx < b.idx;
+}
+
+__device__ __forceinline__ Best warp_best(Best v) {
+#pragma unroll
+  for (int off = 16; off; off >>= 1) {
+    Best o;
+    o.C = __shfl_xor_sync(0xffffffffu, v.C, off);
+    o.T = __shfl_xor_sync(0xffffffffu, v.T, off);
+    o.idx = __shfl_xor_sync(0xffffffffu, v.idx, off);
+    if (better(o.C, o.T, o.idx, v)) v = o;
+  }
+  return v;
+}
+
+// ---- TMA (1-D bulk copy) + mbarrier helpers -------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// ---- the per-thread walk ---------------------------------------------------------------------------------------
+template <int L, int K0P, int NB>
+__device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsigned long long o_begin, unsigned long long o_count,
+                                         float* __restrict__ thr_io, Best* __restrict__ best_io, unsigned* __restrict__ slow_io) {
+  constexpr int NBX = NB ? NB : 1;
+  float thr[L];
+  Best best[L];
+  unsigned slow_steps = 0;
+#pragma unroll
+  for (int l = 0; l < L; l++) { thr[l] = thr_io[l]; best[l] = best_io[l]; }
+  const ReqHdr* h = (const ReqHdr*)sb;
+  const int nsp = h->nslots_pad;
+  const int* s_dem0b = (const int*)(sb + kHdrWords);
+  const int* s_lat = s_dem0b + kDem0bWords;      // [slot][L]
+  const float* s_f = (const float*)(s_lat + nsp * L);
+  const int* s_dem = (const int*)(s_f + nsp);
+  const int* s_be = s_dem + nsp;
+  const int Np = h->n_int, K0 = h->K0, K1 = h->K1, slo = h->slo;
+  const bool conn = h->conn01 != 0;
+  const uint32_t deps0 = h->deps[0] & ~3u, deps1 = h->deps[1] & ~3u;
+
+  // inner tables in registers
+  int d0[K0P][L];
+  float f0[K0P];
+  int dem0b[K0P][NBX];
+#pragma unroll
+  for (int k = 0; k < K0P; k++) {
+#pragma unroll
+    for (int l = 0; l < L; l++) d0[k][l] = s_lat[k * L + l];
+    f0[k] = s_f[k];
+#pragma unroll
+    for (int b = 0; b < NBX; b++) dem0b[k][b] = NB ? s_dem0b[k * 8 + b] : 0;
+  }
+  int cap[NBX];
+#pragma unroll
+  for (int b = 0; b < NBX; b++) cap[b] = h->cap[b];
+
+  // outer state (dynamic indexing -> local memory; touched once per K0*K1 plans)
+  int u[16][L];
+  int Rm[17][L];
+  float Cp[17];
+  int Dp[17][NBX];
+  unsigned char dig[16];
+
+#pragma unroll
+  for (int l = 0; l < L; l++) Rm[Np][l] = slo;
+  Cp[Np] = 1.0f;
+#pragma unroll
+  for (int b = 0; b < NBX; b++) Dp[Np][b] = 0;
+  {
+    unsigned long long o = o_begin;
+    for (int i = 2; i < Np; i++) {
+      const unsigned long long kp = (unsigned long long)h->Kp[i];
+      dig[i] = (unsigned char)(o % kp);
+      o /= kp;
+    }
+  }
+  int top = Np - 1;   // recompute nodes top..2
+  for (;;) {
+    for (int i = top; i >= 2; --i) {
+      const int slot = h->optbase[i] + dig[i];
+      int m[L];
+#pragma unroll
+      for (int l = 0; l < L; l++) m[l] = slo;
+      for (uint32_t dm = h->deps[i]; dm; dm &= dm - 1) {
+        const int j = __ffs(dm) - 1;
+#pragma unroll
+        for (int l = 0; l < L; l++) m[l] = min(m[l], u[j][l]);
+      }
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const int v = m[l] - s_lat[slot * L + l];
+        u[i][l] = v;
+        Rm[i][l] = min(Rm[i + 1][l], v);
+      }
+      Cp[i] = Cp[i + 1] * s_f[slot];
+      if (NB) {
+        const int be = s_be[slot], dm = s_dem[slot];
+#pragma unroll
+        for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0);
+      }
+    }
+    // ---- inputs of the middle loop ----
+    int U1[L], A0p[L], R2[L];
+#pragma unroll
+    for (int l = 0; l < L; l++) { U1[l] = slo; A0p[l] = slo; R2[l] = Rm[2][l]; }
+    for (uint32_t dm = deps1; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
+#pragma unroll
+      for (int l = 0; l < L; l++) U1[l] = min(U1[l], u[j][l]);
+    }
+    for (uint32_t dm = deps0; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
+#pragma unroll
+      for (int l = 0; l < L; l++) A0p[l] = min(A0p[l], u[j][l]);
+    }
+    const float C2 = Cp[2];
+    int D2[NBX];
+#pragma unroll
+    for (int b = 0; b < NBX; b++) D2[b] = Dp[2][b];
+
+    for (int k1 = 0; k1 < K1; k1++) {
+      const int slot1 = K0P + k1;
+      const float C1 = C2 * s_f[slot1];
+      int slackD[NBX];
+      int bad = 0;
+      if (NB) {
+        const int be1 = s_be[slot1], dm1 = s_dem[slot1];
+#pragma unroll
+        for (int b = 0; b < NBX; b++) { slackD[b] = cap[b] - D2[b] - (be1 == b ? dm1 : 0); bad |= slackD[b]; }
+      }
+      int ap[L], um[L];
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const int u1 = U1[l] - s_lat[slot1 * L + l];
+        um[l] = min(R2[l], u1);
+        const int A = conn ? min(A0p[l], u1) : A0p[l];
+        ap[l] = ((um[l] | bad) >= 0) ? A : -1;
+      }
+      // ---- fast path: K0P x L evaluations ----
+      int acc0 = -1, acc1 = -1;
+#pragma unroll
+      for (int k0 = 0; k0 < K0P; k0++) {
+        float C = C1 * f0[k0];
+        if (NB) {
+          int w = 0;
+#pragma unroll
+          for (int b = 0; b < NBX; b++) w |= slackD[b] - dem0b[k0][b];
+          C = __int_as_float(__float_as_int(C) | (w & 0x80000000));
+        }
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+          const int t = ap[l] - d0[k0][l];
+          const float y = C - thr[l];
+          if ((k0 + l) & 1) acc1 &= t | __float_as_int(y);
+          else acc0 &= t | __float_as_int(y);
+        }
+      }
+      if ((acc0 & acc1) >= 0) {
+        // ---- slow path: exact order on this prefix ----
+        slow_steps++;
+        unsigned long long idx1 = h->base_idx + (unsigned long long)k1 * h->stride[1];
+        for (int i = 2; i < Np; i++) idx1 += (unsigned long long)dig[i] * h->stride[i];
+        const unsigned long long stride0 = h->stride[0];
+        for (int k0 = 0; k0 < K0; k0++) {
+          const float C = C1 * s_f[k0];
+          if (NB) {
+            int w = 0;
+#pragma unroll
+            for (int b = 0; b < NBX; b++) w |= slackD[b] - s_dem0b[k0 * 8 + b];
+            if (w < 0) continue;
+          }
+          const unsigned long long idx = idx1 + (unsigned long long)k0 * stride0;
+#pragma unroll
+          for (int l = 0; l < L; l++) {
+            const int t = ap[l] - s_lat[k0 * L + l];
+            if (t < 0 || C < thr[l]) continue;
+            const int T = slo - min(t, um[l]);
+            if (better(C, T, idx, best[l])) {
+              best[l].C = C; best[l].T = T; best[l].idx = idx;
+              thr[l] = C;
+            }
+          }
+        }
+      }
+    }
+    // ---- advance the outer digits ----
+    if (--o_count == 0) break;
+    int i = 2;
+    for (;;) {
+      const int d = dig[i] + 1;
+      if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
+      dig[i] = 0;
+      i++;
+    }
+    top = i;
+  }
+#pragma unroll
+  for (int l = 0; l < L; l++) best_io[l] = best[l];
+  *slow_io += slow_steps;
+}
+
+// ---- winner -> bundle record (S6), one thread per (request, level) ---------------------------------------------
+static __device__ void emit_record(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) {
+  const dyplan_batch& b = a.in;
+  const dyplan_bundle& o = a.out;
+  const int B = b.B, M = b.M;
+  const long long rec = r * a.L + l;
+  if (w.idx == kNoIdx) {
+    o.plan_idx[rec] = kNoIdx;
+    for (int i = 0; i < 16; i++) o.choice[rec * 16 + i] = 0xFF;
+    o.corr[rec] = -1.0f;
+    if (o.corr64) o.corr64[rec] = -1.0;
+    o.lat[rec] = INT32_MAX;
+    for (int bb = 0; bb < B; bb++) o.dem[rec * B + bb] = 0;
+    o.dom_model[rec] = 0xFF;
+    o.status[rec] = DYPLAN_ST_INFEASIBLE;
+    return;
+  }
+  const int n0 = h->n0, N = h->n_orig;
+  unsigned long long idx = w.idx;
+  int D[DYPLAN_MAX_BACKENDS], Dm[DYPLAN_MAX_MODELS];
+  for (int i = 0; i < DYPLAN_MAX_BACKENDS; i++) D[i] = 0;
+  for (int i = 0; i < DYPLAN_MAX_MODELS; i++) Dm[i] = 0;
+  double c = 1.0;
+  for (int n = 0; n < 16; n++) {
+    if (n >= N) { o.choice[rec * 16 + n] = 0xFF; continue; }
+    const int ob = b.opt_off[n0 + n];
+    const unsigned long long K = (unsigned long long)(b.opt_off[n0 + n + 1] - ob);
+    const int k = (int)(idx % K);
+    idx /= K;
+    o.choice[rec * 16 + n] = (uint8_t)k;
+    if ((h->skip_mask >> n) & 1) continue;
+    const int op = ob + k;
+    // definition 4 in fp64, node order, no contraction (matches the plain definition bit for bit)
+    c = __dmul_rn(c, __dsub_rn(1.0, __dmul_rn((double)b.vuln[n0 + n], __dsub_rn(1.0, (double)b.acc[op]))));
+    D[b.backend[op]] += b.demand[op];
+    Dm[b.model[op]] += b.demand[op];
+  }
+  int dmod = 0;
+  for (int m = 1; m < M; m++) if (Dm[m] > Dm[dmod]) dmod = m;   // ties -> lowest id (reading Q13)
+  o.plan_idx[rec] = w.idx;
+  o.corr[rec] = w.C;
+  if (o.corr64) o.corr64[rec] = c;
+  o.lat[rec] = w.T;
+  for (int bb = 0; bb < B; bb++) o.dem[rec * B + bb] = D[bb];
+  o.dom_model[rec] = (uint8_t)dmod;
+  o.status[rec] = DYPLAN_ST_OK;
+}
+
+template <int L, int NB>
+__global__ void __launch_bounds__(kBlock) k_score(const CallArgs a) {
+  __shared__ __align__(16) uint32_t s_blob[kMaxBlobWords];
+  __shared__ Best s_red[L][kBlock / 32];
+  __shared__ unsigned long long s_bar;
+  __shared__ uint32_t s_item, s_req, s_last, s_slow;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const size_t blob_stride = blob_stride_words(L);
+  const uint32_t total_items = a.st->total_items;
+  const unsigned long long pio = a.st->per_item_outer;
+  if (tid == 0) { mbar_init(&s_bar, 1); s_slow = 0; }
+  __syncthreads();
+  uint32_t phase = 0;
+  long long cur_req = -1;
+  unsigned slow_steps = 0;
+
+  for (;;) {
+    if (tid == 0) {
+      const uint32_t it = atomicAdd(&a.st->next_item, 1u);
+      s_item = it;
+      if (it < total_items) {
+        // largest r with item_off[r] <= it
+        long long lo = 0, hi = a.in.R;
+        while (hi - lo > 1) { const long long mid = (lo + hi) >> 1; if (a.item_off[mid] <= it) lo = mid; else hi = mid; }
+        s_req = (uint32_t)lo;
+      }
+    }
+    __syncthreads();
+    const uint32_t item = s_item;
+    if (item >= total_items) break;
+    const long long r = s_req;
+    if (r != cur_req) {
+      const uint32_t* gblob = a.blob + (size_t)r * blob_stride;
+      if (tid == 0) {
+        const int nsp = ((const ReqHdr*)gblob)->nslots_pad;
+        const uint32_t bytes = (uint32_t)(kHdrWords + kDem0bWords + nsp * (L + 3)) * 4u;
+        tma_load_1d(s_blob, gblob, bytes, &s_bar);
+      }
+      mbar_wait(&s_bar, phase);
+      phase ^= 1;
+      cur_req = r;
+    }
+    const ReqHdr* h = (const ReqHdr*)s_blob;
+    const uint32_t first_item = a.item_off[r];
+    const unsigned long long ob = (unsigned long long)(item - first_item) * pio;
+    const unsigned long long oe = min(ob + pio, (unsigned long long)h->outer_total);
+    const unsigned long long len = oe - ob;
+    const unsigned long long per = (len + kBlock - 1) / kBlock;
+    const unsigned long long tb = min(ob + (unsigned long long)tid * per, oe);
+    const unsigned long long te = min(tb + per, oe);
+
+    float thr[L];
+    Best best[L];
+#pragma unroll
+    for (int l = 0; l < L; l++) { thr[l] = __ldcg(&a.gthr[r * L + l]); best[l].C = -1.0f; best[l].T = INT32_MAX; best[l].idx = kNoIdx; }
+    if (te > tb) {
+      switch (h->K0p) {
+        case 2: score_range<L, 2, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        case 4: score_range<L, 4, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        case 6: score_range<L, 6, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        case 8: score_range<L, 8, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        case 12: score_range<L, 12, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        default: score_range<L, 16, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+      }
+    }
+    // ---- block arg-best: warp shuffles, then shared memory, then one record per (item, level) ----
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      const Best v = warp_best(best[l]);
+      if (lane == 0) s_red[l][wid] = v;
+    }
+    __syncthreads();
+    if (tid < L) {
+      Best v = s_red[tid][0];
+      for (int w = 1; w < kBlock / 32; w++) { const Best o = s_red[tid][w]; if (better(o.C, o.T, o.idx, v)) v = o; }
+      Partial p; p.C = v.C; p.T = v.T; p.idx = v.idx;
+      a.partial[(size_t)item * L + tid] = p;
+      if (v.idx != kNoIdx) atomicMax((int*)&a.gthr[r * L + tid], __float_as_int(v.C));
+      __threadfence();
+    }
+    __syncthreads();
+    if (tid == 0) {
+      const uint32_t n_it = a.item_off[r + 1] - first_item;
+      const uint32_t t = atomicAdd(&a.done[r], 1u);
+      s_last = (t == n_it - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last) {
+      // ---- last block of this request: reduce its items' records and emit the bundle (fused K_final) ----
+      __threadfence();
+      const uint32_t n_it = a.item_off[r + 1] - first_item;
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
+        for (uint32_t j = tid; j < n_it; j += kBlock) {
+          const Partial* pp = &a.partial[(size_t)(first_item + j) * L + l];
+          const float4 raw = __ldcg((const float4*)pp);
+          Best o; o.C = raw.x; o.T = __float_as_int(raw.y);
+          o.idx = ((unsigned long long)__float_as_uint(raw.w) << 32) | (unsigned long long)__float_as_uint(raw.z);
+          if (better(o.C, o.T, o.idx, v)) v = o;
+        }
+        v = warp_best(v);
+        if (lane == 0) s_red[l][wid] = v;
+      }
+      __syncthreads();
+      if (tid < L) {
+        Best v = s_red[tid][0];
+        for (int w = 1; w < kBlock / 32; w++) { const Best o = s_red[tid][w]; if (better(o.C, o.T, o.idx, v)) v = o; }
+        emit_record(a, h, r, tid, v);
+      }
+    }
+    __syncthreads();
+  }
+  if (slow_steps) atomicAdd(&s_slow, slow_steps);
+  __syncthreads();
+  if (tid == 0 && s_slow) atomicAdd(&a.st->slow_steps, (unsigned long long)s_slow);
+}
+
+}  // namespace dyplan
+
+// ---- per-L translation unit body ----------------------------------------------------------------------------------
+#ifdef DYPLAN_SCORE_L
+namespace dyplan {
+#define DYPLAN_CAT2(a, b) a##b
+#define DYPLAN_CAT(a, b) DYPLAN_CAT2(a, b)
+cudaError_t DYPLAN_CAT(launch_score_l, DYPLAN_SCORE_L)(const CallArgs& a, int nb_class, int grid, cudaStream_t s) {
+  constexpr int L = DYPLAN_SCORE_L;
+  switch (nb_class) {
+    case 0: k_score<L, 0><<<grid, kBlock, 0, s>>>(a); break;
+    case 2: k_score<L, 2><<<grid, kBlock, 0, s>>>(a); break;
+    case 4: k_score<L, 4><<<grid, kBlock, 0, s>>>(a); break;
+    default: k_score<L, 8><<<grid, kBlock, 0, s>>>(a); break;
+  }
+  return cudaGetLastError();
+}
+int DYPLAN_CAT(score_occupancy_l, DYPLAN_SCORE_L)(int nb_class) {
+  constexpr int L = DYPLAN_SCORE_L;
+  int n = 0;
+  cudaError_t e;
+  switch (nb_class) {
+    case 0: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_score<L, 0>, kBlock, 0); break;
+    case 2: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_score<L, 2>, kBlock, 0); break;
+    case 4: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_score<L, 4>, kBlock, 0); break;
+    default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_score<L, 8>, kBlock, 0); break;
+  }
+  return e == cudaSuccess ? n : -1;
+}
+}  // namespace dyplan
+#endif

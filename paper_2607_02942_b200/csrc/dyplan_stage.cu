@@ -1,0 +1,310 @@
+// dyplan_stage.cu -- K_stage (validate + stage per-request tables) and K_plan (work decomposition).
+// SURVEY.md 8(a) S0; Alg. 1 l.1-8 "coefficient construction" is the paper's counterpart.
+#include "dyplan_internal.cuh"
+
+namespace dyplan {
+
+__device__ __forceinline__ void write_sentinel(const dyplan_bundle& o, long long rec, int B, int status) {
+  o.plan_idx[rec] = kNoIdx;
+  for (int i = 0; i < 16; i++) o.choice[rec * 16 + i] = 0xFF;
+  o.corr[rec] = -1.0f;
+  if (o.corr64) o.corr64[rec] = -1.0;
+  o.lat[rec] = INT32_MAX;
+  for (int b = 0; b < B; b++) o.dem[rec * B + b] = 0;
+  o.dom_model[rec] = 0xFF;
+  o.status[rec] = (uint8_t)status;
+}
+
+__device__ __forceinline__ int k0_class(int k) { return k <= 2 ? 2 : k <= 4 ? 4 : k <= 6 ? 6 : k <= 8 ? 8 : k <= 12 ? 12 : 16; }
+
+// definition 2 (reading Q4): d_l(n,k) = floor(tau * mult / 1000) in int64
+__device__ __forceinline__ long long scaled(int tau, int mult) { return ((long long)tau * (long long)mult) / 1000; }
+
+// f = 1 - v (1 - a) in fp64 without contraction (f = v * r^, r^ = 1 - q)
+__device__ __forceinline__ double factor64(float v, float a) { return __dsub_rn(1.0, __dmul_rn((double)v, __dsub_rn(1.0, (double)a))); }
+
+// One warp per request.
+__global__ void __launch_bounds__(128) k_stage(CallArgs a) {
+  const int lane = threadIdx.x & 31;
+  const long long r = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const dyplan_batch& b = a.in;
+  if (r >= b.R) return;
+  const int L = a.L, B = b.B;
+  const size_t blob_stride = blob_stride_words(L);
+  uint32_t* blob = a.blob + (size_t)r * blob_stride;
+  ReqHdr* h = (ReqHdr*)blob;
+  const int* mult = a.is_replan ? a.mult + (size_t)r * B : a.mult;
+
+  if (lane == 0) a.done[r] = 0;
+  if (lane < L) a.gthr[r * L + lane] = 0.0f;
+
+  // ---- shape checks, in the oracle's order (load_req, validate, dispatched set, size of the free space) ----
+  int st = DYPLAN_ST_OK;
+  const int n0 = b.node_off[r], n1 = b.node_off[r + 1];
+  const int N = n1 - n0;
+  int K[16], o0[16];
+  unsigned long long stride[16];
+#pragma unroll
+  for (int n = 0; n < 16; n++) { K[n] = 1; o0[n] = 0; stride[n] = 0; }
+  if (N < 0 || N > DYPLAN_MAX_NODES || n0 < 0 || n1 > b.NN) st = DYPLAN_ST_INVALID;
+  if (st == DYPLAN_ST_OK) {
+    unsigned long long s = 1;
+#pragma unroll
+    for (int n = 0; n < 16; n++) {
+      if (n < N && st == DYPLAN_ST_OK) {
+        o0[n] = b.opt_off[n0 + n];
+        K[n] = b.opt_off[n0 + n + 1] - o0[n];
+        if (K[n] < 1 || K[n] > DYPLAN_MAX_OPTS || o0[n] < 0 || o0[n] + K[n] > b.KK) { st = DYPLAN_ST_INVALID; K[n] = 1; }
+        else {
+          stride[n] = s;
+          if (s > ((1ull << 60) / (unsigned long long)K[n])) st = DYPLAN_ST_TOO_LARGE;
+          s *= (unsigned long long)K[n];
+        }
+      }
+    }
+  }
+  if (st == DYPLAN_ST_OK) {
+    bool bad = false;
+    for (int i = lane; i < L * B; i += 32) bad |= mult[i] < 0;
+    if (lane == 0) bad |= b.slo_us[r] < 0;
+    if (b.cap && lane < B) bad |= b.cap[r * B + lane] < 0;
+    // per-node fields: lane n
+    int nodeK = 1, nodeo0 = 0;
+#pragma unroll
+    for (int n = 0; n < 16; n++) if (n == lane) { nodeK = K[n]; nodeo0 = o0[n]; }
+    if (lane < N) {
+      const uint32_t pm = b.pred_mask[n0 + lane];
+      bad |= (pm >> lane) != 0;
+      const float v = b.vuln[n0 + lane];
+      bad |= !(v >= 0.0f && v <= 1.0f);
+      for (int k = 0; k < nodeK; k++) {
+        const int o = nodeo0 + k;
+        bad |= b.lat_us[o] < 0 || b.demand[o] < 0;
+        const float ac = b.acc[o];
+        bad |= !(ac >= 0.0f && ac <= 1.0f);
+        bad |= b.backend[o] >= B || b.model[o] >= b.M;
+      }
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    if (!bad) {
+      // reading Q19: sum_n max_k d_l and sum_n max_k demand must fit int32
+      for (int l = 0; l <= L && !bad; l++) {
+        long long mx = 0;
+        if (lane < N)
+          for (int k = 0; k < nodeK; k++) {
+            const int o = nodeo0 + k;
+            const long long d = (l < L) ? scaled(b.lat_us[o], mult[l * B + b.backend[o]]) : (long long)b.demand[o];
+            mx = d > mx ? d : mx;
+          }
+#pragma unroll
+        for (int off = 16; off; off >>= 1) mx += __shfl_xor_sync(0xffffffffu, mx, off);
+        bad |= mx > (long long)INT32_MAX;
+      }
+    }
+    if (bad) st = DYPLAN_ST_INVALID;
+  }
+  uint32_t fmask = 0;
+  if (st == DYPLAN_ST_OK && a.is_replan) {
+    fmask = a.dispatched[r];
+    bool bad = (N < 32) && ((fmask >> N) != 0);
+    if (!bad && lane < N && ((fmask >> lane) & 1)) {
+      int nodeK = 1;
+#pragma unroll
+      for (int n = 0; n < 16; n++) if (n == lane) nodeK = K[n];
+      bad |= a.fixed_choice[n0 + lane] >= nodeK;
+      bad |= (b.pred_mask[n0 + lane] & ~fmask) != 0;   // reading Q11: predecessor-closed
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    if (bad) st = DYPLAN_ST_INVALID;
+  }
+  unsigned long long P = 1;
+  if (st == DYPLAN_ST_OK) {
+#pragma unroll
+    for (int n = 0; n < 16; n++)
+      if (n < N && !((fmask >> n) & 1) && st == DYPLAN_ST_OK) {
+        P *= (unsigned long long)K[n];
+        if (P > (1ull << DYPLAN_MAX_PLANS_LOG2)) st = DYPLAN_ST_TOO_LARGE;
+      }
+  }
+  if (st != DYPLAN_ST_OK) {
+    if (lane == 0) { h->status = st; h->outer_total = 0; h->nslots_pad = 0; h->K0 = 1; h->K1 = 1; }
+    if (lane < L) write_sentinel(a.out, r * L + lane, B, st);
+    return;
+  }
+
+  // ---- internal order ----
+  const int Kfirst = N ? (((fmask >> 0) & 1) ? 1 : K[0]) : 1;
+  int Klast = 1;
+#pragma unroll
+  for (int n = 0; n < 16; n++) if (n == N - 1) Klast = ((fmask >> n) & 1) ? 1 : K[n];
+  const int orient = (N >= 1 && Klast > Kfirst) ? 1 : 0;
+  const int Np = N < 3 ? 3 : N;
+  const bool residual = a.is_replan && (a.flags & DYPLAN_RESIDUAL);
+
+  // lane i < Np describes internal node i
+  int e = -1;
+  if (lane < N) e = orient ? N - 1 - lane : lane;
+  int myK = 1, myo0 = 0; unsigned long long mystride = 0;
+#pragma unroll
+  for (int n = 0; n < 16; n++) if (n == e) { myK = K[n]; myo0 = o0[n]; mystride = stride[n]; }
+  const bool fixed = e >= 0 && ((fmask >> e) & 1);
+  const int fk = fixed ? a.fixed_choice[n0 + e] : 0;
+  const int Kp = (e < 0 || fixed) ? 1 : myK;
+  uint32_t deps = 0;
+  if (e >= 0) {
+    if (!orient) {
+      for (int j = e + 1; j < N; j++) if ((b.pred_mask[n0 + j] >> e) & 1) deps |= 1u << j;
+    } else {
+      const uint32_t pm = b.pred_mask[n0 + e];
+      for (int p = 0; p < e; p++) if ((pm >> p) & 1) deps |= 1u << (N - 1 - p);
+    }
+  }
+  const int K0r = __shfl_sync(0xffffffffu, Kp, 0), K1r = __shfl_sync(0xffffffffu, Kp, 1);
+  const int K0p = k0_class(K0r);
+  const int width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
+  int optbase = width;   // inclusive scan over lanes -> exclusive
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
+  const int nslots = __shfl_sync(0xffffffffu, optbase, 31);
+  optbase -= width;
+  const int nslots_pad = (nslots + 3) & ~3;
+  unsigned long long outer = (lane >= 2 && lane < Np) ? (unsigned long long)Kp : 1ull;
+  unsigned long long base = fixed ? (unsigned long long)fk * mystride : 0ull;
+#pragma unroll
+  for (int off = 16; off; off >>= 1) { outer *= __shfl_xor_sync(0xffffffffu, outer, off); base += __shfl_xor_sync(0xffffffffu, base, off); }
+  const uint32_t deps0 = __shfl_sync(0xffffffffu, deps, 0);
+
+  if (lane == 0) {
+    h->status = DYPLAN_ST_OK; h->n_int = Np; h->n_orig = N; h->orient = orient; h->K0 = K0r; h->K1 = K1r; h->K0p = K0p;
+    h->slo = b.slo_us[r]; h->nslots_pad = nslots_pad; h->n0 = n0; h->conn01 = (deps0 >> 1) & 1;
+    h->skip_mask = residual ? fmask : 0u; h->outer_total = outer; h->base_idx = base;
+    for (int bb = 0; bb < 8; bb++) h->cap[bb] = (b.cap && bb < B) ? b.cap[r * B + bb] : INT32_MAX;
+  }
+  if (lane < 16) {
+    h->Kp[lane] = lane < Np ? Kp : 1;
+    h->deps[lane] = lane < Np ? deps : 0;
+    h->optbase[lane] = lane < Np ? optbase : 0;
+    h->fixk[lane] = fixed ? fk : -1;
+    h->stride[lane] = (lane < Np && !fixed) ? mystride : 0ull;
+  }
+
+  // ---- tables: dem0b [16][8], lat [slot][L], f [slot], dem [slot], be [slot] ----
+  int* t_dem0b = (int*)(blob + kHdrWords);
+  int* t_lat = t_dem0b + kDem0bWords;
+  float* t_f = (float*)(t_lat + nslots_pad * L);
+  int* t_dem = (int*)(t_f + nslots_pad);
+  int* t_be = t_dem + nslots_pad;
+  for (int i = lane; i < kDem0bWords; i += 32) t_dem0b[i] = 0;
+  __syncwarp();
+  for (int s0 = 0; s0 < nslots_pad; s0 += 32) {   // uniform trip count: the body shuffles
+    const int s = s0 + lane;
+    const bool active = s < nslots_pad;
+    // which internal node owns slot s
+    int node = -1, k = 0;
+    for (int i = 0; i < Np; i++) {
+      const int ob = __shfl_sync(0xffffffffu, optbase, i), w = __shfl_sync(0xffffffffu, width, i);
+      if (s >= ob && s < ob + w) { node = i; k = s - ob; }
+    }
+    int ne = -1, nK = 1, no0 = 0, nfix = 0, nfk = 0;
+    for (int i = 0; i < Np; i++) {
+      const int ee = __shfl_sync(0xffffffffu, e, i), kk = __shfl_sync(0xffffffffu, myK, i), oo = __shfl_sync(0xffffffffu, myo0, i);
+      const int ff = __shfl_sync(0xffffffffu, (int)fixed, i), fkk = __shfl_sync(0xffffffffu, fk, i);
+      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; }
+    }
+    int dl[DYPLAN_MAX_LEVELS];
+#pragma unroll
+    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = 0;
+    float f = 1.0f; int dem = 0, be = 0;
+    const bool pad = node < 0 || (node == 0 && k >= K0r);
+    if (pad) {
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = INT32_MAX;
+      f = 0.0f;
+    } else if (ne >= 0 && !(nfix && residual)) {
+      const int o = no0 + (nfix ? nfk : k);
+      be = b.backend[o]; dem = b.demand[o];
+      const int tau = b.lat_us[o];
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) if (l < L) dl[l] = (int)scaled(tau, mult[l * B + be]);
+      f = (float)factor64(b.vuln[n0 + ne], b.acc[o]);
+    }
+    if (active) {
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) if (l < L) t_lat[s * L + l] = dl[l];
+      t_f[s] = f; t_dem[s] = dem; t_be[s] = be;
+      if (node == 0 && !pad) t_dem0b[k * 8 + be] = dem;
+    }
+  }
+}
+
+// Single block: totals, items per request, exclusive scan.
+__global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
+  __shared__ unsigned long long s_sum[1024];
+  __shared__ unsigned long long s_plans[1024];
+  __shared__ uint32_t s_cnt[1024];
+  const int tid = threadIdx.x;
+  const long long R = a.in.R;
+  const size_t blob_stride = blob_stride_words(a.L);
+  const long long chunk = (R + 1023) / 1024;
+  const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
+  unsigned long long so = 0, sp = 0;
+  for (long long r = r0; r < r1; r++) {
+    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+    if (h->status == DYPLAN_ST_OK) { so += h->outer_total; sp += h->outer_total * (unsigned long long)(h->K0 * h->K1); }
+  }
+  s_sum[tid] = so; s_plans[tid] = sp;
+  __syncthreads();
+  for (int off = 512; off; off >>= 1) { if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_plans[tid] += s_plans[tid + off]; } __syncthreads(); }
+  const unsigned long long total_outer = s_sum[0], total_plans = s_plans[0];
+  __syncthreads();
+  // outer indices per work item: a multiple of the block size; ~16K items when there is enough work,
+  // never more than max_items - R extra items.
+  const unsigned long long target = 16384;
+  unsigned long long pio = (total_outer + target - 1) / target;
+  const unsigned long long extra = a.max_items > (unsigned long long)R ? a.max_items - (unsigned long long)R : 1;
+  const unsigned long long need = (total_outer + extra - 1) / extra;
+  if (need > pio) pio = need;
+  pio = ((pio + kBlock - 1) / kBlock) * kBlock;
+  if (pio < (unsigned long long)kBlock) pio = kBlock;
+  uint32_t cnt = 0;
+  for (long long r = r0; r < r1; r++) {
+    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+    if (h->status == DYPLAN_ST_OK) cnt += (uint32_t)((h->outer_total + pio - 1) / pio);
+  }
+  s_cnt[tid] = cnt;
+  __syncthreads();
+  // inclusive scan (Hillis-Steele over 1024 entries)
+  for (int off = 1; off < 1024; off <<= 1) {
+    uint32_t v = tid >= off ? s_cnt[tid - off] : 0;
+    __syncthreads();
+    s_cnt[tid] += v;
+    __syncthreads();
+  }
+  uint32_t run = s_cnt[tid] - cnt;
+  for (long long r = r0; r < r1; r++) {
+    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+    a.item_off[r] = run;
+    if (h->status == DYPLAN_ST_OK) run += (uint32_t)((h->outer_total + pio - 1) / pio);
+  }
+  if (tid == 1023) {
+    a.item_off[R] = s_cnt[1023];
+    CallState* st = a.st;
+    st->total_outer = total_outer; st->total_plans = total_plans; st->per_item_outer = pio; st->slow_steps = 0;
+    st->total_items = s_cnt[1023]; st->next_item = 0; st->mult_invalid = 0; st->pad = 0;
+  }
+}
+
+cudaError_t launch_stage(const CallArgs& a, cudaStream_t s) {
+  const int wpb = 4;
+  const unsigned grid = (unsigned)((a.in.R + wpb - 1) / wpb);
+  if (grid == 0) return cudaSuccess;
+  k_stage<<<grid, wpb * 32, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_plan(const CallArgs& a, cudaStream_t s) {
+  k_plan<<<1, 1024, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace dyplan

@@ -1,0 +1,313 @@
+"""-m gpu: the CUDA path (through the C ABI of include/dyplan.h) against the fp64 oracle, record by record.
+
+Sizes are chosen so the oracle finishes in seconds yet every case spans many work items, several inner
+tiles and a ragged tail.  Full BASELINE.json sizes are covered in test_gpu_full_size.py.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2607_02942_b200 import workloads as wl
+
+from parity import check_records
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dy():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    from paper_2607_02942_b200 import binding
+    ctx = binding.Context(0)
+    yield binding, ctx
+    ctx.close()
+
+
+def gpu_run(dy, w, corr64=True):
+    import torch
+    binding, ctx = dy
+    dw = binding.upload(w, "cuda:0", corr64)
+    binding.launch(ctx, dw)
+    torch.cuda.synchronize()
+    return dw.out.host()
+
+
+def both(dy, orc, w, where):
+    g = gpu_run(dy, w)
+    ref = orc.run(w)
+    c = check_records(orc, w, g, ref, where=where)
+    return g, ref, c
+
+
+# ---- BASELINE.json configs, down-scaled where the oracle needs it --------------------------------------------------
+def test_cfg0_diamond_full(dy, orc):
+    w = wl.make_config(0)
+    g, ref, c = both(dy, orc, w, "cfg0")
+    assert c["records"] == 3
+    assert (ref["status"] == 0).any()
+
+
+def test_cfg1_prefix(dy, orc):
+    w = wl.make_config(1, R=3)      # 3 x 8^8 plans x 4 levels
+    both(dy, orc, w, "cfg1[3]")
+
+
+def test_cfg2_prefix(dy, orc):
+    w = wl.make_config(2, R=24)     # 24 x 8^7 plans x 4 levels, caps
+    both(dy, orc, w, "cfg2[24]")
+
+
+def test_cfg3_prefix_both_flags(dy, orc):
+    w = wl.make_config(3, R=96)
+    # keep the oracle in seconds: drop the 12^7 queries (2 dispatched) from this case
+    keep = [r for r in range(w.batch.R) if bin(int(w.dispatched_mask[r])).count("1") >= 3][:40]
+    w = w.subset(keep)
+    both(dy, orc, w, "cfg3[fixed-in-place]")
+    w.flags = wl.FLAG_RESIDUAL
+    both(dy, orc, w, "cfg3[residual]")
+
+
+def test_cfg4_shape_reduced_nodes(dy, orc):
+    # cfg4's option structure (3 models x 2 verifiers, backend = model, B = 3, 8 levels, caps) at N = 9
+    full = wl.make_config(4, R=2)
+    rng = np.random.default_rng(44)
+    reqs = []
+    for r in range(2):
+        n = 9
+        pm = wl.layered_pred_masks(rng, n, 4, 0.5)
+        a, e = int(full.batch.node_off[r]), int(full.batch.node_off[r]) + n
+        oa, oe = int(full.batch.opt_off[a]), int(full.batch.opt_off[e])
+        K = 6
+        reqs.append(dict(pred_mask=pm, vuln=full.batch.vuln[a:e],
+                         lat=full.batch.lat_us[oa:oe].reshape(n, K), acc=full.batch.acc[oa:oe].reshape(n, K),
+                         demand=full.batch.demand[oa:oe].reshape(n, K), backend=full.batch.backend[oa:oe].reshape(n, K),
+                         model=full.batch.model[oa:oe].reshape(n, K), slo=int(full.batch.slo_us[r] * 0.8),
+                         cap=(full.batch.cap.reshape(-1, 3)[r] * 0.8).astype(np.int32)))
+    b = wl.batch_from_requests(reqs, 3, 3, True)
+    w = wl.Workload(name="cfg4-n9", kind="compile", batch=b, L=8, mult_pm=full.mult_pm)
+    both(dy, orc, w, "cfg4-n9")
+
+
+# ---- ragged, free-form cases --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,L,B,caps", [(1, 1, 1, False), (2, 2, 2, True), (3, 3, 3, True), (4, 4, 2, False),
+                                           (5, 5, 5, True), (6, 6, 2, True), (7, 7, 8, True), (8, 8, 4, False)])
+def test_random_ragged(dy, orc, seed, L, B, caps):
+    w = wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=7, B=B, M=min(B + 1, 8), L=L, caps=caps)
+    both(dy, orc, w, f"ragged(seed={seed})")
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_random_wide_options(dy, orc, seed):
+    # K up to 16 (every inner radix class), few nodes
+    w = wl.random_workload(seed, R=24, nmin=2, nmax=5, kmin=9, kmax=16, B=2, M=3, L=3, caps=True, tool_p=0.0)
+    both(dy, orc, w, f"wide(seed={seed})")
+
+
+@pytest.mark.parametrize("seed", [21, 22])
+def test_random_many_nodes_tool_nodes(dy, orc, seed):
+    # up to 14 nodes, most of them tool nodes (K = 1), arbitrary DAGs
+    w = wl.random_workload(seed, R=12, nmin=10, nmax=14, kmin=2, kmax=3, B=2, M=3, L=2, caps=True, tool_p=0.45,
+                           edge_p=0.3)
+    both(dy, orc, w, f"deep(seed={seed})")
+
+
+@pytest.mark.parametrize("seed,flags", [(31, wl.FLAG_FIXED_IN_PLACE), (32, wl.FLAG_RESIDUAL),
+                                        (33, wl.FLAG_FIXED_IN_PLACE), (34, wl.FLAG_RESIDUAL)])
+def test_random_replan(dy, orc, seed, flags):
+    w = wl.random_replan_workload(seed, R=48, nmin=1, nmax=8, kmin=1, kmax=6, B=3, M=3, caps=True, flags=flags)
+    g, ref, c = both(dy, orc, w, f"replan(seed={seed})")
+    # the cases the paper singles out: nothing left to choose / everything left to choose
+    nd = np.array([bin(int(m)).count("1") for m in w.dispatched_mask])
+    nn = np.array([w.batch.n_nodes(r) for r in range(w.batch.R)])
+    assert (nd == nn).any() and (nd == 0).any()
+
+
+def test_slo_sweep_monotone_and_infeasible(dy, orc):
+    # SLO below the smallest possible T => INFEASIBLE at every level; huge SLO, no caps => separable optimum
+    w = wl.random_workload(41, R=6, nmin=4, nmax=6, kmin=3, kmax=5, B=2, M=2, L=3, caps=False)
+    w.batch.slo_us[:] = 0
+    w.batch.lat_us[:] = np.maximum(w.batch.lat_us, 1)
+    g, ref, _ = both(dy, orc, w, "slo=0")
+    assert (g["status"] == 1).all()
+    w.batch.slo_us[:] = 2**31 - 1
+    g, ref, _ = both(dy, orc, w, "slo=max")
+    assert (g["status"] == 0).all()
+    for r in range(w.batch.R):
+        a, e = w.batch.node_off[r], w.batch.node_off[r + 1]
+        best = 1.0
+        for n in range(a, e):
+            f = 1.0 - float(w.batch.vuln[n]) * (1.0 - w.batch.acc[w.batch.opt_off[n]: w.batch.opt_off[n + 1]].astype(np.float64))
+            best *= f.max()
+        assert abs(g["corr64"][r * 3] - best) <= 1e-12 * best     # PIN8 on the GPU path
+
+
+def test_all_vulnerabilities_zero_tie_break(dy, orc):
+    # C == 1 for every plan: the winner is the (T asc, idx asc) minimum, bit-exact index (order 7)
+    w = wl.random_workload(42, R=8, nmin=3, nmax=6, kmin=2, kmax=6, B=2, M=2, L=4, caps=True)
+    w.batch.vuln[:] = 0.0
+    g, ref, c = both(dy, orc, w, "v=0")
+    assert c["within_tol"] == 0
+    ok = ref["status"] == 0
+    assert (g["plan_idx"][ok] == ref["plan_idx"][ok]).all()
+    assert (g["corr"][ok] == 1.0).all()
+
+
+def test_duplicate_options_exact_ties(dy, orc):
+    # backend-only variants tie in C (quality does not depend on the backend): T then idx decides
+    w = wl.make_config(1, R=2)
+    b = w.batch
+    b.acc[:] = np.round(b.acc * 8) / 8          # few distinct accuracies -> many exact C ties
+    b.vuln[:] = np.round(b.vuln * 4) / 4
+    g, ref, c = both(dy, orc, w, "ties")
+
+
+# ---- malformed inputs: per-request status, the rest of the batch still compiles ------------------------
+def test_invalid_requests_are_isolated(dy, orc):
+    w = wl.random_workload(51, R=12, nmin=3, nmax=6, kmin=2, kmax=5, B=2, M=3, L=2, caps=True, tool_p=0.0)
+    b = w.batch
+    n0 = b.node_off
+    b.pred_mask[n0[1] + 1] |= np.uint32(1 << 2)            # predecessor with a larger index
+    b.vuln[n0[3]] = np.nan                                 # missing vulnerability is not zero
+    b.acc[b.opt_off[n0[5]]] = 1.5
+    b.lat_us[b.opt_off[n0[7] + 1]] = -3
+    b.backend[b.opt_off[n0[9]]] = 7                        # >= B
+    b.slo_us[10] = -1
+    g, ref, _ = both(dy, orc, w, "invalid")
+    st = g["status"].reshape(b.R, 2)
+    for r in (1, 3, 5, 7, 9, 10):
+        assert (st[r] == 2).all(), r
+    for r in (0, 2, 4, 6, 8, 11):
+        assert (st[r] != 2).all(), r
+
+
+def test_latency_overflow_is_invalid(dy, orc):
+    w = wl.random_workload(52, R=3, nmin=4, nmax=5, kmin=2, kmax=3, B=2, M=2, L=2, caps=False, tool_p=0.0)
+    o = w.batch.opt_off[w.batch.node_off[1]]
+    w.batch.lat_us[o] = 2**31 - 1                           # x multiplier >= 1000 per mille, summed: > INT32_MAX
+    g, ref, _ = both(dy, orc, w, "overflow")
+    assert (g["status"].reshape(3, 2)[1] == 2).all()
+
+
+def test_replan_dispatched_set_must_be_predecessor_closed(dy, orc):
+    w = wl.random_replan_workload(53, R=6, nmin=5, nmax=6, kmin=2, kmax=4, B=2, M=2, caps=False, tool_p=0.0)
+    b = w.batch
+    # chain 0 -> 1 in request 2, dispatch node 1 but not node 0
+    b.pred_mask[b.node_off[2] + 1] = 1
+    w.dispatched_mask[2] = 0b10
+    w.fixed_choice[b.node_off[4]] = 15                      # fixed choice >= K_n
+    w.dispatched_mask[4] |= 1
+    g, ref, _ = both(dy, orc, w, "replan-invalid")
+    assert g["status"][2] == 2 and g["status"][4] == 2
+
+
+def test_plan_space_too_large(dy, orc):
+    # 16 nodes x 16 options = 2^64 plans: TOO_LARGE, not a hang
+    n, K = 16, 16
+    req = dict(pred_mask=[0] * n, vuln=np.full(n, 0.5, np.float32), lat=np.full((n, K), 10, np.int32),
+               acc=np.full((n, K), 0.5, np.float32), demand=np.full((n, K), 1, np.int32),
+               backend=np.zeros((n, K), np.uint8), model=np.zeros((n, K), np.uint8), slo=1000, cap=[100])
+    small = dict(req)
+    small.update(pred_mask=[0] * 2, vuln=req["vuln"][:2], lat=req["lat"][:2, :2], acc=req["acc"][:2, :2],
+                 demand=req["demand"][:2, :2], backend=req["backend"][:2, :2], model=req["model"][:2, :2])
+    b = wl.batch_from_requests([req, small], 1, 1, True)
+    w = wl.Workload(name="huge", kind="compile", batch=b, L=1, mult_pm=np.array([1000], np.int32))
+    g, ref, _ = both(dy, orc, w, "too-large")
+    assert g["status"][0] == 3 and g["status"][1] == 0
+
+
+def test_empty_batch_and_empty_request(dy, orc):
+    import torch
+    binding, ctx = dy
+    w = wl.random_workload(54, R=3, nmin=2, nmax=3, kmin=2, kmax=3, B=2, M=2, L=2, caps=False)
+    e = wl.Workload(name="empty", kind="compile", batch=wl.batch_from_requests([], 2, 2, False), L=2,
+                    mult_pm=w.mult_pm)
+    dw = binding.upload(e)
+    binding.launch(ctx, dw)          # R = 0: a no-op that returns OK
+    torch.cuda.synchronize()
+    # a request with zero nodes has exactly one (empty) plan: C = 1, T = 0
+    b = w.batch
+    b2 = wl.Batch(R=2, B=b.B, M=b.M, node_off=np.array([0, 0, b.node_off[1]], np.int32),
+                  opt_off=b.opt_off[: b.node_off[1] + 1].copy(), pred_mask=b.pred_mask[: b.node_off[1]].copy(),
+                  vuln=b.vuln[: b.node_off[1]].copy(), lat_us=b.lat_us[: b.opt_off[b.node_off[1]]].copy(),
+                  acc=b.acc[: b.opt_off[b.node_off[1]]].copy(), demand=b.demand[: b.opt_off[b.node_off[1]]].copy(),
+                  backend=b.backend[: b.opt_off[b.node_off[1]]].copy(), model=b.model[: b.opt_off[b.node_off[1]]].copy(),
+                  slo_us=np.array([5, b.slo_us[0]], np.int32), cap=None)
+    w2 = wl.Workload(name="empty-req", kind="compile", batch=b2, L=2, mult_pm=w.mult_pm)
+    g, ref, _ = both(dy, orc, w2, "empty-req")
+    assert (g["status"][:2] == 0).all() and (g["corr"][:2] == 1.0).all() and (g["lat"][:2] == 0).all()
+
+
+# ---- the *_host entry points and select ----------------------------------------------------------------------------
+def test_host_calls_equal_device_calls(dy, orc):
+    binding, ctx = dy
+    for w in (wl.random_workload(61, R=30, nmin=2, nmax=6, kmin=2, kmax=6, B=3, M=3, L=3, caps=True),
+              wl.random_replan_workload(62, R=30, nmin=2, nmax=7, kmin=2, kmax=5, B=2, M=3, caps=True)):
+        g = gpu_run(dy, w)
+        h, h2d, d2h = binding.run_host(ctx, w)
+        for k in g:
+            assert np.array_equal(g[k], h[k]), k
+        assert h2d > 0 and d2h > 0
+
+
+@pytest.mark.parametrize("seed", [71, 72, 73])
+def test_select_parity(dy, orc, seed):
+    import torch
+    binding, ctx = dy
+    L, B = 4, 3
+    w = wl.random_workload(seed, R=200, nmin=1, nmax=8, kmin=1, kmax=4, B=B, M=3, L=L, caps=True, slo_q=0.3)
+    w.batch.vuln[w.batch.node_off[5]] = np.nan     # one invalid request -> variant -1
+    dw = binding.upload(w)
+    binding.launch(ctx, dw)
+    torch.cuda.synchronize()
+    g = dw.out.host()
+    rng = np.random.default_rng(seed)
+    for trial in range(4):
+        live = rng.integers(1000, 4001, size=B).astype(np.int32) if trial else np.asarray(w.mult_pm[:B], np.int32)
+        dlive = torch.from_numpy(live).cuda()
+        variant = torch.full((w.batch.R,), -7, dtype=torch.int32, device="cuda")
+        res = binding.alloc_bundle(w.batch.R, 1, B, "cuda:0")
+        ctx.dyplan_select(dw.batch, dw.out, L, dlive, variant, res)
+        torch.cuda.synchronize()
+        ref = orc.select(w.batch, L, g["choice"], g["status"], live)
+        v = variant.cpu().numpy()
+        assert np.array_equal(v, ref["variant"])
+        rs = res.host()
+        pick = v >= 0
+        assert np.array_equal(rs["lat"][pick].astype(np.int64), ref["lat"][pick])
+        assert np.allclose(rs["corr64"][pick], ref["corr"][pick], rtol=1e-12, atol=0)
+        assert np.array_equal(rs["status"][pick] == 0, ref["feasible"][pick] == 1)
+        assert (rs["status"][~pick] != 0).all() and v[5] == -1
+        # the re-scored record is a consistent plan of the stored bundle
+        for r in np.nonzero(pick)[0][:50]:
+            rec = r * L + v[r]
+            assert np.array_equal(rs["choice"].reshape(-1, 16)[r], g["choice"].reshape(-1, 16)[rec])
+            assert rs["plan_idx"][r] == g["plan_idx"][rec]
+            assert np.array_equal(rs["dem"].reshape(-1, B)[r], g["dem"].reshape(-1, B)[rec])
+            assert rs["dom_model"][r] == g["dom_model"][rec]
+        if trial == 0:
+            # PIN14 on the GPU path: under level 0's own multipliers variant 0 re-scores to its stored T
+            ok0 = g["status"].reshape(-1, L)[:, 0] == 0
+            assert (v[ok0] >= 0).all()
+        # host entry point gives the same answer
+        vh = np.full(w.batch.R, -9, np.int32)
+        hb = binding.make_batch(w.batch, None)
+        hbundle = binding.bundle_from_host(g, w.batch.R, L, B, None)
+        ctx.dyplan_select_host(hb, hbundle, L, live, vh, None)
+        assert np.array_equal(vh, v)
+
+
+def test_api_argument_errors(dy):
+    binding, ctx = dy
+    w = wl.random_workload(81, R=2, nmin=2, nmax=3, kmin=2, kmax=3, B=2, M=2, L=2, caps=False)
+    dw = binding.upload(w)
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_compile(dw.batch, 9, dw.mult, dw.out)          # L over the limit
+    assert e.value.code == binding.ERR_LIMIT
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_compile(dw.batch, 2, None, dw.out)             # NULL multipliers
+    assert e.value.code == binding.ERR_NULL
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_replan(dw.batch, dw.mult, dw.mult, dw.mult, 2, dw.out)   # unknown flag
+    assert e.value.code == binding.ERR_ARG
