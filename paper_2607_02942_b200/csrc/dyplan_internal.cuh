@@ -9,6 +9,7 @@
 namespace dyplan {
 
 constexpr int kBlock = 128;          // threads per scoring block
+constexpr int kMinBlocks = 4;        // resident scoring blocks per SM the register allocation is bounded for
 constexpr int kHdrWords = 120;       // ReqHdr size in 4-byte words (multiple of 4 -> 16-byte aligned tables)
 constexpr int kMaxSlots = 16 * 16 + 4;  // option slots of one request incl. dummies, padded to 4
 constexpr int kDem0bWords = 16 * 8;  // per-backend demand of the inner node's options [k0][b]

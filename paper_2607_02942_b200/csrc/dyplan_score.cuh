@@ -17,7 +17,7 @@
 
 namespace dyplan {
 
-struct Best {
+struct __align__(16) Best {
   float C;
   int32_t T;
   unsigned long long idx;
@@ -70,15 +70,23 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t pari
 }
 
 // ---- the per-thread walk ---------------------------------------------------------------------------------------
-template <int L, int K0P, int NB>
+// Loop nest of one thread over its range of outer indices (digits of internal nodes >= 2, odometer order):
+//   heavy step  (a digit >= 3 changed)  generic slack DP of nodes top..3 over local-memory arrays, then the
+//                                       "node-2 context": everything node 2 / 1 / 0 need from nodes >= 3
+//   light step  (digit 2)               u2, running minimum, inputs of the middle loop, C2, D2; thresholds re-read
+//   middle loop (digit 1)               one fused add-min per level gives a'_l, the slack bound of node 0
+//   inner block (digit 0, unrolled)     the 3-instruction screen per (plan, level); tables in registers
+//   slow path   (a lane saw a candidate) exact re-walk of that K0-wide group, order 7, incumbent update
+// Thresholds are shared by the block: s_thr[l] = bits of the best C found so far (any thread, plus what other
+// blocks published in gthr when the item started), s_thrm[l] = bits of its float predecessor.  The screen tests
+// the exact sign of C1*f0 - pred(thr) with one FFMA: fl(C1*f0) >= thr implies C1*f0 > pred(thr), so no plan that
+// ties or beats the incumbent in fp32 is ever screened out.
+template <int L, int K0P, int NB, bool CONN>
 __device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsigned long long o_begin, unsigned long long o_count,
-                                         float* __restrict__ thr_io, Best* __restrict__ best_io, unsigned* __restrict__ slow_io) {
+                                         volatile int* s_thr, volatile int* s_thrm, Best* s_best, int* g_thr,
+                                         unsigned* __restrict__ slow_io) {
   constexpr int NBX = NB ? NB : 1;
-  float thr[L];
-  Best best[L];
   unsigned slow_steps = 0;
-#pragma unroll
-  for (int l = 0; l < L; l++) { thr[l] = thr_io[l]; best[l] = best_io[l]; }
   const ReqHdr* h = (const ReqHdr*)sb;
   const int nsp = h->nslots_pad;
   const int* s_dem0b = (const int*)(sb + kHdrWords);
@@ -86,9 +94,10 @@ __device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsign
   const float* s_f = (const float*)(s_lat + nsp * L);
   const int* s_dem = (const int*)(s_f + nsp);
   const int* s_be = s_dem + nsp;
-  const int Np = h->n_int, K0 = h->K0, K1 = h->K1, slo = h->slo;
-  const bool conn = h->conn01 != 0;
-  const uint32_t deps0 = h->deps[0] & ~3u, deps1 = h->deps[1] & ~3u;
+  const int Np = h->n_int, K0 = h->K0, K1 = h->K1, K2 = h->Kp[2], slo = h->slo;
+  const int ob2 = h->optbase[2];
+  const uint32_t deps0 = h->deps[0], deps1 = h->deps[1], deps2 = h->deps[2];
+  const bool d0has2 = (deps0 >> 2) & 1, d1has2 = (deps1 >> 2) & 1;
 
   // inner tables in registers
   int d0[K0P][L];
@@ -106,13 +115,12 @@ __device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsign
 #pragma unroll
   for (int b = 0; b < NBX; b++) cap[b] = h->cap[b];
 
-  // outer state (dynamic indexing -> local memory; touched once per K0*K1 plans)
+  // state of the nodes >= 3 (dynamic indexing -> local memory; touched once per K2*K1*K0 plans)
   int u[16][L];
   int Rm[17][L];
   float Cp[17];
   int Dp[17][NBX];
   unsigned char dig[16];
-
 #pragma unroll
   for (int l = 0; l < L; l++) Rm[Np][l] = slo;
   Cp[Np] = 1.0f;
@@ -126,9 +134,14 @@ __device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsign
       o /= kp;
     }
   }
-  int top = Np - 1;   // recompute nodes top..2
+  int k2 = dig[2];
+  int top = Np - 1;   // recompute nodes top..3
+  // node-2 context
+  int X2[L], Rm3[L], U1r[L], A0r[L], D3[NBX];
+  float C3;
   for (;;) {
-    for (int i = top; i >= 2; --i) {
+    // ---- heavy step ----
+    for (int i = top; i >= 3; --i) {
       const int slot = h->optbase[i] + dig[i];
       int m[L];
 #pragma unroll
@@ -151,103 +164,146 @@ __device__ __noinline__ void score_range(const uint32_t* __restrict__ sb, unsign
         for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0);
       }
     }
-    // ---- inputs of the middle loop ----
-    int U1[L], A0p[L], R2[L];
 #pragma unroll
-    for (int l = 0; l < L; l++) { U1[l] = slo; A0p[l] = slo; R2[l] = Rm[2][l]; }
-    for (uint32_t dm = deps1; dm; dm &= dm - 1) {
+    for (int l = 0; l < L; l++) { X2[l] = slo; U1r[l] = slo; A0r[l] = slo; Rm3[l] = Rm[3][l]; }
+    for (uint32_t dm = deps2; dm; dm &= dm - 1) {
       const int j = __ffs(dm) - 1;
 #pragma unroll
-      for (int l = 0; l < L; l++) U1[l] = min(U1[l], u[j][l]);
+      for (int l = 0; l < L; l++) X2[l] = min(X2[l], u[j][l]);
     }
-    for (uint32_t dm = deps0; dm; dm &= dm - 1) {
+    for (uint32_t dm = deps1 & ~7u; dm; dm &= dm - 1) {
       const int j = __ffs(dm) - 1;
 #pragma unroll
-      for (int l = 0; l < L; l++) A0p[l] = min(A0p[l], u[j][l]);
+      for (int l = 0; l < L; l++) U1r[l] = min(U1r[l], u[j][l]);
     }
-    const float C2 = Cp[2];
-    int D2[NBX];
+    for (uint32_t dm = deps0 & ~7u; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
 #pragma unroll
-    for (int b = 0; b < NBX; b++) D2[b] = Dp[2][b];
+      for (int l = 0; l < L; l++) A0r[l] = min(A0r[l], u[j][l]);
+    }
+    C3 = Cp[3];
+#pragma unroll
+    for (int b = 0; b < NBX; b++) D3[b] = Dp[3][b];
 
-    for (int k1 = 0; k1 < K1; k1++) {
-      const int slot1 = K0P + k1;
-      const float C1 = C2 * s_f[slot1];
-      int slackD[NBX];
-      int bad = 0;
-      if (NB) {
-        const int be1 = s_be[slot1], dm1 = s_dem[slot1];
-#pragma unroll
-        for (int b = 0; b < NBX; b++) { slackD[b] = cap[b] - D2[b] - (be1 == b ? dm1 : 0); bad |= slackD[b]; }
-      }
-      int ap[L], um[L];
+    for (;;) {
+      // ---- light step: node 2 takes option k2 ----
+      const int slot2 = ob2 + k2;
+      int R2[L], U1[L], A0q[L];
+      float thrmf[L];
 #pragma unroll
       for (int l = 0; l < L; l++) {
-        const int u1 = U1[l] - s_lat[slot1 * L + l];
-        um[l] = min(R2[l], u1);
-        const int A = conn ? min(A0p[l], u1) : A0p[l];
-        ap[l] = ((um[l] | bad) >= 0) ? A : -1;
+        const int u2 = X2[l] - s_lat[slot2 * L + l];
+        R2[l] = min(Rm3[l], u2);
+        U1[l] = d1has2 ? min(U1r[l], u2) : U1r[l];
+        const int a0 = d0has2 ? min(A0r[l], u2) : A0r[l];
+        A0q[l] = R2[l] < 0 ? R2[l] : a0;          // a node >= 2 already misses the SLO: every bound below goes negative
+        thrmf[l] = __int_as_float(s_thrm[l]);
       }
-      // ---- fast path: K0P x L evaluations ----
-      int acc0 = -1, acc1 = -1;
+      const float C2 = C3 * s_f[slot2];
+      int D2[NBX];
+      if (NB) {
+        const int be2 = s_be[slot2], dm2 = s_dem[slot2];
 #pragma unroll
-      for (int k0 = 0; k0 < K0P; k0++) {
-        float C = C1 * f0[k0];
+        for (int b = 0; b < NBX; b++) D2[b] = D3[b] + (be2 == b ? dm2 : 0);
+      }
+
+      for (int k1 = 0; k1 < K1; k1++) {
+        const int slot1 = K0P + k1;
+        const float C1 = C2 * s_f[slot1];
+        int slackD[NBX];
+        int bad = 0;
         if (NB) {
-          int w = 0;
+          const int be1 = s_be[slot1], dm1 = s_dem[slot1];
 #pragma unroll
-          for (int b = 0; b < NBX; b++) w |= slackD[b] - dem0b[k0][b];
-          C = __int_as_float(__float_as_int(C) | (w & 0x80000000));
+          for (int b = 0; b < NBX; b++) { slackD[b] = cap[b] - D2[b] - (be1 == b ? dm1 : 0); bad |= slackD[b]; }
         }
+        const float C1s = NB ? __int_as_float(__float_as_int(C1) | (bad & 0x80000000)) : C1;
+        int ap[L];
 #pragma unroll
         for (int l = 0; l < L; l++) {
-          const int t = ap[l] - d0[k0][l];
-          const float y = C - thr[l];
-          if ((k0 + l) & 1) acc1 &= t | __float_as_int(y);
-          else acc0 &= t | __float_as_int(y);
+          const int lat1 = s_lat[slot1 * L + l];
+          if (CONN) ap[l] = min(U1[l] - lat1, A0q[l]);                    // one VIADDMNMX
+          else { const int u1 = U1[l] - lat1; ap[l] = u1 < 0 ? u1 : A0q[l]; }
         }
-      }
-      if ((acc0 & acc1) >= 0) {
-        // ---- slow path: exact order on this prefix ----
-        slow_steps++;
-        unsigned long long idx1 = h->base_idx + (unsigned long long)k1 * h->stride[1];
-        for (int i = 2; i < Np; i++) idx1 += (unsigned long long)dig[i] * h->stride[i];
-        const unsigned long long stride0 = h->stride[0];
-        for (int k0 = 0; k0 < K0; k0++) {
-          const float C = C1 * s_f[k0];
-          if (NB) {
-            int w = 0;
+        // ---- screen: K0P x L evaluations ----
+        int acc0 = -1, acc1 = -1;
 #pragma unroll
-            for (int b = 0; b < NBX; b++) w |= slackD[b] - s_dem0b[k0 * 8 + b];
-            if (w < 0) continue;
+        for (int k0 = 0; k0 < K0P; k0++) {
+          float Ck = C1s;
+          if (NB) {
+            int w = slackD[0] - dem0b[k0][0];
+#pragma unroll
+            for (int b = 1; b < NBX; b++) w = min(w, slackD[b] - dem0b[k0][b]);
+            Ck = __int_as_float(__float_as_int(C1s) | (w & 0x80000000));
           }
-          const unsigned long long idx = idx1 + (unsigned long long)k0 * stride0;
 #pragma unroll
           for (int l = 0; l < L; l++) {
-            const int t = ap[l] - s_lat[k0 * L + l];
-            if (t < 0 || C < thr[l]) continue;
-            const int T = slo - min(t, um[l]);
-            if (better(C, T, idx, best[l])) {
-              best[l].C = C; best[l].T = T; best[l].idx = idx;
-              thr[l] = C;
-            }
+            const int t = ap[l] - d0[k0][l];
+            const float y = __fmaf_rn(Ck, f0[k0], -thrmf[l]);
+            if ((k0 + l) & 1) acc1 &= t | __float_as_int(y);
+            else acc0 &= t | __float_as_int(y);
           }
         }
-      }
-    }
-    // ---- advance the outer digits ----
-    if (--o_count == 0) break;
-    int i = 2;
-    for (;;) {
-      const int d = dig[i] + 1;
-      if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
-      dig[i] = 0;
-      i++;
-    }
-    top = i;
-  }
+        if (__builtin_expect((acc0 & acc1) >= 0, 0)) {
+          // ---- slow path: exact order on this group ----
+          slow_steps++;
+          unsigned long long idx1 = h->base_idx + (unsigned long long)k1 * h->stride[1] + (unsigned long long)k2 * h->stride[2];
+          for (int i = 3; i < Np; i++) idx1 += (unsigned long long)dig[i] * h->stride[i];
+          const unsigned long long stride0 = h->stride[0];
+          if (bad >= 0) {
+            for (int k0 = 0; k0 < K0; k0++) {
+              const float C = __fmul_rn(C1, s_f[k0]);
+              if (NB) {
+                int w = 0;
 #pragma unroll
-  for (int l = 0; l < L; l++) best_io[l] = best[l];
+                for (int b = 0; b < NBX; b++) w |= slackD[b] - s_dem0b[k0 * 8 + b];
+                if (w < 0) continue;
+              }
+              const unsigned long long idx = idx1 + (unsigned long long)k0 * stride0;
+#pragma unroll
+              for (int l = 0; l < L; l++) {
+                const int t = ap[l] - s_lat[k0 * L + l];
+                const int tb = s_thr[l];
+                if (t < 0 || C < __int_as_float(tb)) continue;
+                const int um = min(R2[l], U1[l] - s_lat[slot1 * L + l]);
+                const int T = slo - min(t, um);
+                Best* bp = &s_best[l * kBlock];
+                const Best cur = *bp;
+                if (better(C, T, idx, cur)) {
+                  Best nb; nb.C = C; nb.T = T; nb.idx = idx;
+                  *bp = nb;
+                  const int cb = __float_as_int(C);
+                  if (cb > tb) {
+                    atomicMax((int*)&s_thr[l], cb);
+                    atomicMax((int*)&s_thrm[l], cb > 0 ? cb - 1 : (int)0x80000001);
+                    atomicMax(&g_thr[l], cb);
+                  }
+                }
+              }
+            }
+          }
+#pragma unroll
+          for (int l = 0; l < L; l++) thrmf[l] = __int_as_float(s_thrm[l]);
+        }
+      }
+      // ---- advance ----
+      if (--o_count == 0) goto done;
+      if (++k2 < K2) continue;
+      k2 = 0;
+      break;
+    }
+    {
+      int i = 3;
+      for (;;) {
+        const int d = dig[i] + 1;
+        if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
+        dig[i] = 0;
+        i++;
+      }
+      top = i;
+    }
+  }
+done:
   *slow_io += slow_steps;
 }
 
@@ -299,10 +355,19 @@ static __device__ void emit_record(const CallArgs& a, const ReqHdr* h, long long
   o.status[rec] = DYPLAN_ST_OK;
 }
 
+template <int L, int K0P, int NB>
+__device__ __forceinline__ void score_dispatch(bool conn, const uint32_t* sb, unsigned long long b, unsigned long long n, volatile int* s_thr,
+                                               volatile int* s_thrm, Best* s_best, int* g_thr, unsigned* slow) {
+  if (conn) score_range<L, K0P, NB, true>(sb, b, n, s_thr, s_thrm, s_best, g_thr, slow);
+  else score_range<L, K0P, NB, false>(sb, b, n, s_thr, s_thrm, s_best, g_thr, slow);
+}
+
 template <int L, int NB>
-__global__ void __launch_bounds__(kBlock) k_score(const CallArgs a) {
+__global__ void __launch_bounds__(kBlock, kMinBlocks) k_score(const CallArgs a) {
   __shared__ __align__(16) uint32_t s_blob[kMaxBlobWords];
+  __shared__ __align__(16) Best s_best[L * kBlock];   // [level][thread]: the thread's incumbent (touched by the slow path only)
   __shared__ Best s_red[L][kBlock / 32];
+  __shared__ __align__(16) int s_thr[8], s_thrm[8];
   __shared__ unsigned long long s_bar;
   __shared__ uint32_t s_item, s_req, s_last, s_slow;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -342,6 +407,15 @@ __global__ void __launch_bounds__(kBlock) k_score(const CallArgs a) {
       cur_req = r;
     }
     const ReqHdr* h = (const ReqHdr*)s_blob;
+    int* g_thr = (int*)a.gthr + r * L;
+    if (tid < L) {
+      const int b = __ldcg(&g_thr[tid]);            // what every block has published so far (bits of a float >= 0)
+      s_thr[tid] = b;
+      s_thrm[tid] = b > 0 ? b - 1 : (int)0x80000001;  // bits of the float just below it
+    }
+#pragma unroll
+    for (int l = 0; l < L; l++) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; s_best[l * kBlock + tid] = e; }
+    __syncthreads();
     const uint32_t first_item = a.item_off[r];
     const unsigned long long ob = (unsigned long long)(item - first_item) * pio;
     const unsigned long long oe = min(ob + pio, (unsigned long long)h->outer_total);
@@ -350,24 +424,21 @@ __global__ void __launch_bounds__(kBlock) k_score(const CallArgs a) {
     const unsigned long long tb = min(ob + (unsigned long long)tid * per, oe);
     const unsigned long long te = min(tb + per, oe);
 
-    float thr[L];
-    Best best[L];
-#pragma unroll
-    for (int l = 0; l < L; l++) { thr[l] = __ldcg(&a.gthr[r * L + l]); best[l].C = -1.0f; best[l].T = INT32_MAX; best[l].idx = kNoIdx; }
     if (te > tb) {
+      const bool conn = h->conn01 != 0;
       switch (h->K0p) {
-        case 2: score_range<L, 2, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
-        case 4: score_range<L, 4, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
-        case 6: score_range<L, 6, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
-        case 8: score_range<L, 8, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
-        case 12: score_range<L, 12, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
-        default: score_range<L, 16, NB>(s_blob, tb, te - tb, thr, best, &slow_steps); break;
+        case 2: score_dispatch<L, 2, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
+        case 4: score_dispatch<L, 4, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
+        case 6: score_dispatch<L, 6, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
+        case 8: score_dispatch<L, 8, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
+        case 12: score_dispatch<L, 12, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
+        default: score_dispatch<L, 16, NB>(conn, s_blob, tb, te - tb, s_thr, s_thrm, s_best + tid, g_thr, &slow_steps); break;
       }
     }
     // ---- block arg-best: warp shuffles, then shared memory, then one record per (item, level) ----
 #pragma unroll
     for (int l = 0; l < L; l++) {
-      const Best v = warp_best(best[l]);
+      const Best v = warp_best(s_best[l * kBlock + tid]);
       if (lane == 0) s_red[l][wid] = v;
     }
     __syncthreads();
@@ -376,7 +447,7 @@ __global__ void __launch_bounds__(kBlock) k_score(const CallArgs a) {
       for (int w = 1; w < kBlock / 32; w++) { const Best o = s_red[tid][w]; if (better(o.C, o.T, o.idx, v)) v = o; }
       Partial p; p.C = v.C; p.T = v.T; p.idx = v.idx;
       a.partial[(size_t)item * L + tid] = p;
-      if (v.idx != kNoIdx) atomicMax((int*)&a.gthr[r * L + tid], __float_as_int(v.C));
+      if (v.idx != kNoIdx) atomicMax(&g_thr[tid], __float_as_int(v.C));
       __threadfence();
     }
     __syncthreads();

@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     if (pad) {
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = INT32_MAX;
-      f = 0.0f;
+      f = -1.0f;   // a padding option can never tie or beat an incumbent: C1 * f <= 0
     } else if (ne >= 0 && !(nfix && residual)) {
       const int o = no0 + (nfix ? nfk : k);
       be = b.backend[o]; dem = b.demand[o];
