@@ -152,6 +152,7 @@ typedef struct {
   uint64_t evals;       /* (plan, level) evaluations = sum_r plans_r * L                                          */
   uint64_t work_items;  /* (request, plan-range) work items the scorer processed                                  */
   uint64_t slow_steps;  /* inner blocks that took the exact (slow) path                                           */
+  uint64_t fast_requests; /* requests scored by the fp32 kernel (the others went to the int32 kernel)             */
   int32_t launches;     /* kernels launched by the last call                                                      */
   int32_t sm_count;     /* SMs of the device                                                                      */
   float score_ms;       /* device time of the scoring kernel of the last call (CUDA events on `stream`)           */

@@ -26,6 +26,24 @@ int score_occupancy_l7(int);
 int score_occupancy_l8(int);
 static const score_launcher_t kLaunch[8] = {launch_score_l1, launch_score_l2, launch_score_l3, launch_score_l4,
                                             launch_score_l5, launch_score_l6, launch_score_l7, launch_score_l8};
+cudaError_t launch_fscore_l1(const CallArgs&, int, cudaStream_t);
+cudaError_t launch_fscore_l2(const CallArgs&, int, cudaStream_t);
+cudaError_t launch_fscore_l3(const CallArgs&, int, cudaStream_t);
+cudaError_t launch_fscore_l4(const CallArgs&, int, cudaStream_t);
+cudaError_t launch_fscore_l6(const CallArgs&, int, cudaStream_t);
+cudaError_t launch_fscore_l8(const CallArgs&, int, cudaStream_t);
+int fscore_occupancy_l1();
+int fscore_occupancy_l2();
+int fscore_occupancy_l3();
+int fscore_occupancy_l4();
+int fscore_occupancy_l6();
+int fscore_occupancy_l8();
+// indexed by the real level count - 1 (levels 5 and 7 run in the 6- and 8-level instantiations)
+static const fscore_launcher_t kFLaunch[8] = {launch_fscore_l1, launch_fscore_l2, launch_fscore_l3, launch_fscore_l4,
+                                              launch_fscore_l6, launch_fscore_l6, launch_fscore_l8, launch_fscore_l8};
+typedef int (*focc_fn_t)();
+static const focc_fn_t kFOcc[8] = {fscore_occupancy_l1, fscore_occupancy_l2, fscore_occupancy_l3, fscore_occupancy_l4,
+                                   fscore_occupancy_l6, fscore_occupancy_l6, fscore_occupancy_l8, fscore_occupancy_l8};
 typedef int (*occ_fn_t)(int);
 static const occ_fn_t kOcc[8] = {score_occupancy_l1, score_occupancy_l2, score_occupancy_l3, score_occupancy_l4,
                                  score_occupancy_l5, score_occupancy_l6, score_occupancy_l7, score_occupancy_l8};
@@ -44,11 +62,12 @@ struct dyplan_ctx {
   cudaError_t last_err = cudaSuccess;
   char errbuf[256] = {0};
   // scratch
-  DevBuf blob, item_off, done, gthr, partial, state;
+  DevBuf blob, item_off, done, gthr, partial, state;   // item_off holds both classes' offset arrays
   // staging for the *_host calls: one device arena, one pinned-or-not host side is the caller's
   DevBuf arena;
   // occupancy cache [L-1][nb index]
   int occ[8][4];
+  int focc[8];
   // last call
   cudaStream_t last_stream = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -111,7 +130,7 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
     delete ctx;
     return DYPLAN_ERR_CUDA;
   }
-  for (int i = 0; i < 8; i++) for (int j = 0; j < 4; j++) ctx->occ[i][j] = 0;
+  for (int i = 0; i < 8; i++) { for (int j = 0; j < 4; j++) ctx->occ[i][j] = 0; ctx->focc[i] = 0; }
   *out = ctx;
   return DYPLAN_OK;
 }
@@ -168,9 +187,24 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   CK(cudaSetDevice(ctx->device));
 
   const size_t R = (size_t)in->R;
-  const uint32_t max_items = (uint32_t)(R + 32768);
+  const int nbc = nb_class_of(in->B, in->cap != nullptr);
+  int& occ = ctx->occ[L - 1][nb_index(nbc)];
+  if (occ <= 0) {
+    occ = kOcc[L - 1](nbc);
+    if (occ <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
+  }
+  int& focc = ctx->focc[L - 1];
+  if (focc <= 0) {
+    focc = kFOcc[L - 1]();
+    if (focc <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
+  }
+  // persistent grids: every block resident, work pulled from device counters
+  const int grid = ctx->sm_count * occ;
+  const int fgrid = ctx->sm_count * focc;
+  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * 24u;
+  const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * (target_items_f > 32768u ? target_items_f : 32768u);
   if ((rc = ensure(ctx, ctx->blob, R * blob_stride_words(L) * 4))) return rc;
-  if ((rc = ensure(ctx, ctx->item_off, (R + 1) * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->item_off, 2 * (R + 1) * 4))) return rc;
   if ((rc = ensure(ctx, ctx->done, R * 4))) return rc;
   if ((rc = ensure(ctx, ctx->gthr, R * L * 4))) return rc;
   if ((rc = ensure(ctx, ctx->partial, (size_t)max_items * L * sizeof(Partial)))) return rc;
@@ -180,25 +214,20 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   memset(&a, 0, sizeof(a));
   a.in = *in; a.out = *out; a.L = L; a.mult = mult; a.dispatched = dispatched; a.fixed_choice = fixed_choice;
   a.flags = flags; a.is_replan = is_replan ? 1 : 0;
-  a.blob = (uint32_t*)ctx->blob.p; a.item_off = (uint32_t*)ctx->item_off.p; a.done = (uint32_t*)ctx->done.p;
+  a.blob = (uint32_t*)ctx->blob.p; a.item_off = (uint32_t*)ctx->item_off.p; a.item_off_f = a.item_off + (R + 1);
+  a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f;
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
   a.max_items = max_items;
 
-  const int nbc = nb_class_of(in->B, in->cap != nullptr);
-  int& occ = ctx->occ[L - 1][nb_index(nbc)];
-  if (occ <= 0) {
-    occ = kOcc[L - 1](nbc);
-    if (occ <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
-  }
-  const int grid = ctx->sm_count * occ;   // persistent: every block resident, work pulled from a device counter
 
   CK(launch_stage(a, stream));
   CK(launch_plan(a, stream));
   CK(cudaEventRecord(ctx->ev0, stream));
-  CK(kLaunch[L - 1](a, nbc, grid, stream));
+  CK(kFLaunch[L - 1](a, fgrid, stream));      // fp32 scorer: requests of the fast class
+  CK(kLaunch[L - 1](a, nbc, grid, stream));   // int32 scorer: the rest (exits at once when it has no work items)
   CK(cudaEventRecord(ctx->ev1, stream));
   ctx->have_events = true;
-  ctx->last_launches = 3;
+  ctx->last_launches = 4;
   return DYPLAN_OK;
 }
 
@@ -247,7 +276,8 @@ int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
     CK(cudaMemcpy(&st, ctx->state.p, sizeof(st), cudaMemcpyDeviceToHost));
     out->plans = st.total_plans;
     out->evals = st.total_plans * (uint64_t)ctx->last_L;
-    out->work_items = st.total_items;
+    out->work_items = (uint64_t)st.total_items + st.total_items_f;
+    out->fast_requests = st.fast_requests;
     out->slow_steps = st.slow_steps;
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));

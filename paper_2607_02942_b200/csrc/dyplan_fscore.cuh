@@ -1,0 +1,387 @@
+// dyplan_fscore.cuh -- K_fscore: enumerate + score + arg-best for requests of the fast class,
+// one template per padded level count L.  Included by dyplan_fscore_l<L>.cu with DYPLAN_FSCORE_L defined.
+//
+// Same walk as k_score (dyplan_score.cuh), but
+//   * the slack DP of Eq.(3) runs on exact fp32 integers (k_stage admits a request only when every slack, latency
+//     and demand sum stays below 2^22), because on sm_100a FADD/FMUL/FFMA issue at 1 warp-instruction/clk/SMSP
+//     while IADD3/LOP3/VIADDMNMX/IMAD issue at 0.5 (measured, profiles/r1c_m0_pipe_rates.md);
+//   * the work item belongs to one WARP, not one block: no block barrier anywhere in the loop;
+//   * per (plan, level) the screen is two FMA-pipe instructions and half an ALU-pipe instruction:
+//         x = sat(ap1_l - d0[k0][l])          FADD.SAT   1 iff node 0 (hence every node) meets the SLO at level l
+//         z = x * P - pred(thr_l)             FFMA       > 0 iff feasible and C32(plan) >= incumbent of level l
+//         zmax = max3(zmax, z, z')            FMNMX3     one per two evaluations
+//     with P = C1 * f0[k0] (one FMUL per plan; with caps P is also multiplied by x_cap = sat(slackD_g + 1 - dem0[k0]),
+//     node 0's options being laid out in one slot group per backend).  A group whose zmax > 0 is re-walked by the
+//     exact slow path (order 7 with T and the canonical index), which updates the lane's incumbent.
+#pragma once
+#include "dyplan_common.cuh"
+
+namespace dyplan {
+
+template <int L>
+struct __align__(16) FWarpShared {
+  uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
+  Best best[L * 32];               // [level][lane]: the lane's incumbent (touched by the slow path only)
+  int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
+  unsigned long long bar;          // mbarrier of the TMA copy
+  unsigned long long pad;
+};
+
+// Loop nest of one lane over its range of outer indices (digits of internal nodes >= 2, odometer order):
+//   heavy step  (a digit >= 3 changed)  slack DP of nodes top..3 over local-memory arrays, node-2 context, thresholds
+//                                       refreshed from what every warp published in g_thr
+//   light step  (digit 2)               u2, running minimum, inputs of the middle loop, C2, cap slack
+//   middle loop (digit 1)               ap1_l = min(A0q1_l, (U1_l + 1 - d1_l) * S01): slack bound (+1) of node 0
+//   inner block (digit 0, unrolled)     the screen; tables in registers
+//   slow path                           exact re-walk of the K0P-wide group
+template <int L, int K0P, int NB>
+__device__ __noinline__ void frange(const uint32_t* __restrict__ sb, unsigned long long o_begin, unsigned long long o_count,
+                                    int* w_thr, Best* my_best, int* g_thr, const int Lr, unsigned* __restrict__ slow_io) {
+  constexpr int NBX = NB ? NB : 1;
+  constexpr int G = NB ? K0P / NB : K0P;
+  unsigned slow_steps = 0;
+  const ReqHdr* h = (const ReqHdr*)sb;
+  const int nsp = h->nslots_pad;
+  const float* s_nlat = (const float*)(sb + kHdrWords);   // [slot][L], negated durations
+  const float* s_f = s_nlat + nsp * L;
+  const float* s_dem = s_f + nsp;
+  const int* s_be = (const int*)(s_dem + nsp);
+  const unsigned long long* s_idxc = (const unsigned long long*)(s_be + nsp);
+  const float* s_dem1b = (const float*)(s_idxc + nsp);   // [k1][8], caps only
+  const int Np = h->n_int, K1 = h->K1, K2 = h->Kp[2];
+  const int ob2 = h->optbase[2];
+  const float slo = h->slo_f, S01 = h->S01, rS01 = 1.0f / h->S01, big12 = h->big12, big02 = h->big02;
+  const uint32_t deps0 = h->deps[0], deps1 = h->deps[1], deps2 = h->deps[2];
+
+  // inner tables in registers
+  float nd0[K0P][L], f0[K0P], ndem0[K0P];
+#pragma unroll
+  for (int k = 0; k < K0P; k++) {
+#pragma unroll
+    for (int l = 0; l < L; l++) nd0[k][l] = s_nlat[k * L + l];
+    f0[k] = s_f[k];
+    ndem0[k] = NB ? -s_dem[k] : 0.0f;
+  }
+  float capf[NBX];
+#pragma unroll
+  for (int b = 0; b < NBX; b++) capf[b] = h->capf[b];
+
+  // state of the nodes >= 3 (dynamic indexing -> local memory; touched once per K2*K1*K0 plans)
+  float u[16][L];
+  float Rm[17][L];
+  float Cp[17];
+  float Dp[17][NBX];
+  unsigned char dig[16];
+#pragma unroll
+  for (int l = 0; l < L; l++) Rm[Np][l] = slo;
+  Cp[Np] = 1.0f;
+#pragma unroll
+  for (int b = 0; b < NBX; b++) Dp[Np][b] = 0.0f;
+  {
+    unsigned long long o = o_begin;
+    for (int i = 2; i < Np; i++) {
+      const unsigned long long kp = (unsigned long long)h->Kp[i];
+      dig[i] = (unsigned char)(o % kp);
+      o /= kp;
+    }
+  }
+  int k2 = dig[2];
+  int top = Np - 1;   // recompute nodes top..3
+  float X2[L], Rm3[L], U1r[L], A0r[L], D3[NBX];
+  float C3;
+  float nthrm[L];   // -pred(thr_l): the screen's addend
+  for (;;) {
+    // ---- heavy step ----
+    for (int i = top; i >= 3; --i) {
+      const int slot = h->optbase[i] + dig[i];
+      float m[L];
+#pragma unroll
+      for (int l = 0; l < L; l++) m[l] = slo;
+      for (uint32_t dm = h->deps[i]; dm; dm &= dm - 1) {
+        const int j = __ffs(dm) - 1;
+#pragma unroll
+        for (int l = 0; l < L; l++) m[l] = fminf(m[l], u[j][l]);
+      }
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const float v = m[l] + s_nlat[slot * L + l];
+        u[i][l] = v;
+        Rm[i][l] = fminf(Rm[i + 1][l], v);
+      }
+      Cp[i] = Cp[i + 1] * s_f[slot];
+      if (NB) {
+        const int be = s_be[slot];
+        const float dm = s_dem[slot];
+#pragma unroll
+        for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0.0f);
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < L; l++) { X2[l] = slo; U1r[l] = slo; A0r[l] = slo; Rm3[l] = Rm[3][l]; }
+    for (uint32_t dm = deps2; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
+#pragma unroll
+      for (int l = 0; l < L; l++) X2[l] = fminf(X2[l], u[j][l]);
+    }
+    for (uint32_t dm = deps1 & ~7u; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
+#pragma unroll
+      for (int l = 0; l < L; l++) U1r[l] = fminf(U1r[l], u[j][l]);
+    }
+    for (uint32_t dm = deps0 & ~7u; dm; dm &= dm - 1) {
+      const int j = __ffs(dm) - 1;
+#pragma unroll
+      for (int l = 0; l < L; l++) A0r[l] = fminf(A0r[l], u[j][l]);
+    }
+    C3 = Cp[3];
+#pragma unroll
+    for (int b = 0; b < NBX; b++) D3[b] = Dp[3][b];
+    // thresholds: take what the other warps of this request have published meanwhile
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      const int g = l < Lr ? __ldcg(&g_thr[l]) : 0;
+      int t = ((volatile int*)w_thr)[l];
+      if (g > t) { atomicMax(&w_thr[l], g); t = g; }
+      nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
+    }
+
+    for (;;) {
+      // ---- light step: node 2 takes option k2 ----
+      const int slot2 = ob2 + k2;
+      float R2[L], U1pS[L], A0q1[L];
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const float u2 = X2[l] + s_nlat[slot2 * L + l];
+        R2[l] = fminf(Rm3[l], u2);
+        const float U1 = fminf(U1r[l], u2 + big12);
+        const float a0 = fminf(A0r[l], u2 + big02);
+        A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
+        U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
+      }
+      const float C2 = C3 * s_f[slot2];
+      float sD2[NBX];   // cap slack + 1 before nodes 1 and 0
+      if (NB) {
+        const int be2 = s_be[slot2];
+        const float dm2 = s_dem[slot2];
+#pragma unroll
+        for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
+      }
+
+      for (int k1 = 0; k1 < K1; k1++) {
+        const int slot1 = K0P + k1;
+        float C1 = C2 * s_f[slot1];
+        float s1[NBX];
+        if (NB) {
+          float smin = kBigF;
+#pragma unroll
+          for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - s_dem1b[k1 * 8 + b]; smin = fminf(smin, s1[b]); }
+          C1 *= __saturatef(smin);   // a backend is already over its cap: no plan of this group can be a candidate
+        }
+        float ap1[L];
+#pragma unroll
+        for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
+        // ---- screen: K0P x L evaluations ----
+        float zm = 0.0f;
+#pragma unroll
+        for (int k0 = 0; k0 < K0P; k0++) {
+          float P = C1 * f0[k0];
+          if (NB) P *= __saturatef(s1[k0 / G] + ndem0[k0]);
+          float z[L];
+#pragma unroll
+          for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, nthrm[l]);
+#pragma unroll
+          for (int l = 0; l + 1 < L; l += 2) zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
+          if (L & 1) zm = fmaxf(zm, z[L - 1]);
+        }
+        if (__builtin_expect(zm > 0.0f, 0)) {
+          // ---- slow path: exact order on this group ----
+          slow_steps++;
+          unsigned long long idx1 = h->base_idx + s_idxc[slot1] + s_idxc[slot2];
+          for (int i = 3; i < Np; i++) idx1 += s_idxc[h->optbase[i] + dig[i]];
+#pragma unroll
+          for (int g = 0; g < NBX; g++) {
+            for (int p = 0; p < G; p++) {
+              const int k0 = g * G + p;
+              float P = __fmul_rn(C1, s_f[k0]);
+              if (NB) P = __fmul_rn(P, __saturatef(s1[g] - s_dem[k0]));
+              if (!(P > 0.0f)) continue;
+              const unsigned long long idx = idx1 + s_idxc[k0];
+#pragma unroll
+              for (int l = 0; l < L; l++) {
+                const float t1 = ap1[l] + s_nlat[k0 * L + l];   // slack + 1 of node 0's path
+                if (!(t1 >= 1.0f)) continue;
+                const int tb = ((volatile int*)w_thr)[l];
+                if (P < __int_as_float(tb)) continue;
+                const float u1p = fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]) * rS01;   // slack + 1 of node 1
+                const float ms1 = fminf(fminf(t1, u1p), R2[l] + 1.0f);                  // least slack + 1
+                const int T = (int)((slo + 1.0f) - ms1);
+                Best* bp = &my_best[l * 32];
+                const Best cur = *bp;
+                if (better(P, T, idx, cur)) {
+                  Best nb; nb.C = P; nb.T = T; nb.idx = idx;
+                  *bp = nb;
+                  const int cb = __float_as_int(P);
+                  if (cb > tb) { atomicMax(&w_thr[l], cb); if (l < Lr) atomicMax(&g_thr[l], cb); }
+                }
+              }
+            }
+          }
+#pragma unroll
+          for (int l = 0; l < L; l++) {
+            const int t = ((volatile int*)w_thr)[l];
+            nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
+          }
+        }
+      }
+      // ---- advance ----
+      if (--o_count == 0) goto done;
+      if (++k2 < K2) continue;
+      k2 = 0;
+      break;
+    }
+    {
+      int i = 3;
+      for (;;) {
+        const int d = dig[i] + 1;
+        if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
+        dig[i] = 0;
+        i++;
+      }
+      top = i;
+    }
+  }
+done:
+  *slow_io += slow_steps;
+}
+
+template <int L>
+__global__ void __launch_bounds__(kFastWarps * 32, 4) k_fscore(const CallArgs a) {
+  __shared__ FWarpShared<L> s_w[kFastWarps];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  FWarpShared<L>* ws = &s_w[wid];
+  const int Lr = a.L;                                   // real level count (<= L)
+  const size_t blob_stride = blob_stride_words(Lr);
+  const uint32_t total_items = a.st->total_items_f;
+  const uint32_t rec_base = a.st->total_items;          // partial records of the wide class come first
+  const unsigned long long pif = a.st->per_item_outer_f;
+  if (lane == 0) mbar_init(&ws->bar, 1);
+  __syncwarp();
+  uint32_t phase = 0;
+  long long cur_req = -1;
+  unsigned slow_steps = 0;
+
+  for (;;) {
+    uint32_t item = 0;
+    if (lane == 0) item = atomicAdd(&a.st->next_item_f, 1u);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= total_items) break;
+    long long r;
+    {   // largest r with item_off_f[r] <= item (every lane searches: uniform, L2-resident)
+      long long lo = 0, hi = a.in.R;
+      while (hi - lo > 1) { const long long mid = (lo + hi) >> 1; if (__ldg(&a.item_off_f[mid]) <= item) lo = mid; else hi = mid; }
+      r = lo;
+    }
+    if (r != cur_req) {
+      const uint32_t* gblob = a.blob + (size_t)r * blob_stride;
+      __syncwarp();
+      if (lane == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const uint32_t words = (uint32_t)__ldg(&((const ReqHdr*)gblob)->blob_words);
+        tma_load_1d(ws->blob, gblob, words * 4u, &ws->bar);
+      }
+      mbar_wait(&ws->bar, phase);
+      phase ^= 1;
+      cur_req = r;
+    }
+    const ReqHdr* h = (const ReqHdr*)ws->blob;
+    int* g_thr = (int*)a.gthr + r * Lr;
+    if (lane < 8) ws->thr[lane] = lane < Lr ? __ldcg(&g_thr[lane]) : 0x40000000;   // padded levels: 2.0f, never admitted
+#pragma unroll
+    for (int l = 0; l < L; l++) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; ws->best[l * 32 + lane] = e; }
+    __syncwarp();
+    const uint32_t first_item = __ldg(&a.item_off_f[r]);
+    const unsigned long long ob = (unsigned long long)(item - first_item) * pif;
+    const unsigned long long oe = min(ob + pif, (unsigned long long)h->outer_total);
+    const unsigned long long len = oe - ob;
+    const unsigned long long per = (len + 31) / 32;
+    const unsigned long long tb = min(ob + (unsigned long long)lane * per, oe);
+    const unsigned long long te = min(tb + per, oe);
+
+    if (te > tb) {
+      const unsigned long long n = te - tb;
+      Best* mb = ws->best + lane;
+      switch (h->nbc * 32 + h->K0p) {
+#define DYPLAN_FCASE(NB_, K_) case NB_ * 32 + K_: frange<L, K_, NB_>(ws->blob, tb, n, ws->thr, mb, g_thr, Lr, &slow_steps); break;
+        DYPLAN_FCASE(0, 2) DYPLAN_FCASE(0, 4) DYPLAN_FCASE(0, 6) DYPLAN_FCASE(0, 8) DYPLAN_FCASE(0, 12) DYPLAN_FCASE(0, 16)
+        DYPLAN_FCASE(2, 2) DYPLAN_FCASE(2, 4) DYPLAN_FCASE(2, 6) DYPLAN_FCASE(2, 8) DYPLAN_FCASE(2, 12) DYPLAN_FCASE(2, 16)
+        DYPLAN_FCASE(3, 6) DYPLAN_FCASE(3, 12)
+        DYPLAN_FCASE(4, 4) DYPLAN_FCASE(4, 8) DYPLAN_FCASE(4, 16)
+        DYPLAN_FCASE(8, 8) DYPLAN_FCASE(8, 16)
+#undef DYPLAN_FCASE
+        default: break;   // k_stage never stages another shape for this class
+      }
+    }
+    __syncwarp();
+    // ---- warp arg-best per level (shuffles); lane l keeps level l ----
+    Best mine; mine.C = -1.0f; mine.T = INT32_MAX; mine.idx = kNoIdx;
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      const Best v = warp_best(ws->best[l * 32 + lane]);
+      if (lane == l) mine = v;
+    }
+    if (lane < Lr) {
+      Partial p; p.C = mine.C; p.T = mine.T; p.idx = mine.idx;
+      a.partial[(size_t)(rec_base + item) * Lr + lane] = p;
+      if (mine.idx != kNoIdx) atomicMax(&g_thr[lane], __float_as_int(mine.C));
+      __threadfence();
+    }
+    __syncwarp();
+    const uint32_t n_it = __ldg(&a.item_off_f[r + 1]) - first_item;
+    uint32_t last = 0;
+    if (lane == 0) last = (atomicAdd(&a.done[r], 1u) == n_it - 1) ? 1u : 0u;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (last) {
+      // ---- last warp of this request: reduce its items' records and emit the bundle (fused K_final) ----
+      __threadfence();
+      for (int l = 0; l < Lr; l++) {
+        Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
+        for (uint32_t j = lane; j < n_it; j += 32) {
+          const Partial* pp = &a.partial[(size_t)(rec_base + first_item + j) * Lr + l];
+          const float4 raw = __ldcg((const float4*)pp);
+          Best o; o.C = raw.x; o.T = __float_as_int(raw.y);
+          o.idx = ((unsigned long long)__float_as_uint(raw.w) << 32) | (unsigned long long)__float_as_uint(raw.z);
+          if (better(o.C, o.T, o.idx, v)) v = o;
+        }
+        v = warp_best(v);
+        if (lane == l) mine = v;
+      }
+      if (lane < Lr) emit_record(a, h, r, lane, mine);
+    }
+    __syncwarp();
+  }
+  slow_steps += __shfl_xor_sync(0xffffffffu, slow_steps, 16);
+  slow_steps += __shfl_xor_sync(0xffffffffu, slow_steps, 8);
+  slow_steps += __shfl_xor_sync(0xffffffffu, slow_steps, 4);
+  slow_steps += __shfl_xor_sync(0xffffffffu, slow_steps, 2);
+  slow_steps += __shfl_xor_sync(0xffffffffu, slow_steps, 1);
+  if (lane == 0 && slow_steps) atomicAdd(&a.st->slow_steps, (unsigned long long)slow_steps);
+}
+
+}  // namespace dyplan
+
+// ---- per-L translation unit body ----------------------------------------------------------------------------------
+#ifdef DYPLAN_FSCORE_L
+namespace dyplan {
+#define DYPLAN_CAT2(a, b) a##b
+#define DYPLAN_CAT(a, b) DYPLAN_CAT2(a, b)
+cudaError_t DYPLAN_CAT(launch_fscore_l, DYPLAN_FSCORE_L)(const CallArgs& a, int grid, cudaStream_t s) {
+  k_fscore<DYPLAN_FSCORE_L><<<grid, kFastWarps * 32, 0, s>>>(a);
+  return cudaGetLastError();
+}
+int DYPLAN_CAT(fscore_occupancy_l, DYPLAN_FSCORE_L)() {
+  int n = 0;
+  const cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_fscore<DYPLAN_FSCORE_L>, kFastWarps * 32, 0);
+  return e == cudaSuccess ? n : -1;
+}
+}  // namespace dyplan
+#endif

@@ -18,6 +18,12 @@ constexpr int kMaxBlobWords = kHdrWords + kDem0bWords + kMaxSlots * (DYPLAN_MAX_
 // part is ever written or read, so the stride costs address space, not traffic.
 __host__ __device__ inline size_t blob_stride_words(int L) { return (size_t)kHdrWords + kDem0bWords + (size_t)kMaxSlots * (size_t)(L + 3); }
 constexpr uint64_t kNoIdx = ~0ull;
+constexpr int kClassWide = 0;        // int32 slack DP (k_score): any request the ABI admits
+constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): every latency / demand sum below 2^22, tables <= kFastBlobWords
+constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
+constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
+constexpr float kBigF = 16777216.0f; // 2^24
+__host__ __device__ inline int level_class(int L) { return L <= 4 ? L : (L <= 6 ? 6 : 8); }
 
 // Per-request staged problem in "internal" node order.  Internal node 0 is the innermost
 // enumeration digit, node 1 the middle digit, nodes >= 2 the outer digits.  deps(i) only holds nodes j > i, so
@@ -41,7 +47,15 @@ struct ReqHdr {
   int32_t Kp[16];        // enumerated radix per internal node (1 for pinned / dummy nodes)
   uint32_t deps[16];     // dependency mask per internal node (internal indices, all > i)
   int32_t optbase[16];   // first table slot of internal node i
-  int32_t fixk[16];      // unused (reserved)
+  // --- fields of the float ("fast") scorer; zero for requests of the wide class ---
+  int32_t klass;         // kClassWide or kClassFast
+  int32_t nbc;           // cap class of the fast scorer: 0 (no caps) or 2/3/4/8 backend groups of node 0's slots
+  int32_t Lp;            // level count padded to the scorer's template class (1,2,3,4,6,8)
+  float slo_f;           // min(SLO, longest possible T): every slack is an exact fp32 integer
+  float S01;             // 1 if internal node 1 is in deps(0), else 2^24 (turns "u1 >= 0" into a bound that never binds)
+  float big12, big02;    // 0 if internal node 2 is in deps(1) / deps(0), else 2^24
+  int32_t blob_words;    // words of this request's staged blob (header + tables)
+  float capf[8];         // min(cap, largest possible demand) per backend (+big when absent)
   unsigned long long stride[16];   // canonical stride of internal node i (0 for dummies / pinned nodes)
 };
 static_assert(sizeof(ReqHdr) == kHdrWords * 4, "ReqHdr layout");
@@ -57,11 +71,14 @@ struct __align__(16) Partial {
 struct CallState {
   unsigned long long total_outer;   // sum over valid requests of outer_total
   unsigned long long total_plans;   // sum over valid requests of enumerated plans
-  unsigned long long per_item_outer;
+  unsigned long long per_item_outer;   // wide class: outer indices per (block) work item
+  unsigned long long per_item_outer_f; // fast class: outer indices per (warp) work item
   unsigned long long slow_steps;
-  uint32_t total_items;
-  uint32_t next_item;               // dynamic work counter
-  uint32_t mult_invalid;            // a multiplier was negative
+  uint32_t total_items;             // wide class
+  uint32_t next_item;               // wide class: dynamic work counter
+  uint32_t total_items_f;           // fast class
+  uint32_t next_item_f;
+  uint32_t fast_requests;           // requests staged for the fp32 scorer
   uint32_t pad;
 };
 
@@ -76,12 +93,14 @@ struct CallArgs {                   // passed by value to the kernels
   int32_t is_replan;
   // scratch
   uint32_t* blob;                   // staged requests
-  uint32_t* item_off;               // [R+1]
+  uint32_t* item_off;               // [R+1] wide class
+  uint32_t* item_off_f;             // [R+1] fast class (partial records of fast items follow the wide ones)
   uint32_t* done;                   // [R] ticket counters
   float* gthr;                      // [R*L] published best C per (request, level)
   Partial* partial;                 // [max_items * L]
   CallState* st;
-  uint32_t max_items;
+  uint32_t max_items;               // bound on wide items + fast items
+  uint32_t target_items_f;          // fast class: work items to aim for (a multiple of the resident warps)
 };
 
 
@@ -89,6 +108,7 @@ struct CallArgs {                   // passed by value to the kernels
 cudaError_t launch_stage(const CallArgs& a, cudaStream_t s);
 cudaError_t launch_plan(const CallArgs& a, cudaStream_t s);
 typedef cudaError_t (*score_launcher_t)(const CallArgs& a, int nb_class, int grid, cudaStream_t s);
+typedef cudaError_t (*fscore_launcher_t)(const CallArgs& a, int grid, cudaStream_t s);
 cudaError_t launch_score(const CallArgs& a, int grid, cudaStream_t s);
 int score_blocks_per_sm(int L, int nb_class);
 struct SelectArgs {

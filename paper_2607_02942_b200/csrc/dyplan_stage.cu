@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
 
   // ---- shape checks, in the oracle's order (load_req, validate, dispatched set, size of the free space) ----
   int st = DYPLAN_ST_OK;
+  long long sum_lat = 0, sum_dem = 0;   // largest possible T over the levels / largest possible total demand
   const int n0 = b.node_off[r], n1 = b.node_off[r + 1];
   const int N = n1 - n0;
   int K[16], o0[16];
@@ -99,6 +100,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
 #pragma unroll
         for (int off = 16; off; off >>= 1) mx += __shfl_xor_sync(0xffffffffu, mx, off);
         bad |= mx > (long long)INT32_MAX;
+        if (l < L) sum_lat = mx > sum_lat ? mx : sum_lat; else sum_dem = mx;
       }
     }
     if (bad) st = DYPLAN_ST_INVALID;
@@ -160,41 +162,106 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     }
   }
   const int K0r = __shfl_sync(0xffffffffu, Kp, 0), K1r = __shfl_sync(0xffffffffu, Kp, 1);
-  const int K0p = k0_class(K0r);
-  const int width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
+
+  // ---- scorer class: the fp32 scorer takes a request when every slack and demand sum is an exact
+  // fp32 integer, node 0's options fit its backend-grouped slot layout and the tables fit its shared-memory window ----
+  const int Lp = level_class(L);
+  const bool has_caps = b.cap != nullptr;
+  const int nbc = !has_caps ? 0 : (B <= 2 ? 2 : (B == 3 ? 3 : (B == 4 ? 4 : 8)));
+  // node 0's candidate options: its K options, or the pinned one
+  const int e0 = __shfl_sync(0xffffffffu, e, 0), K0all = __shfl_sync(0xffffffffu, myK, 0), o00 = __shfl_sync(0xffffffffu, myo0, 0);
+  const int fixed0 = __shfl_sync(0xffffffffu, (int)fixed, 0), fk0 = __shfl_sync(0xffffffffu, fk, 0);
+  int G = 0;
+  if (nbc && e0 >= 0) {
+    int cnt[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) cnt[i] = 0;
+    for (int k = 0; k < K0all; k++) {
+      if (fixed0 && k != fk0) continue;
+      const int be = (fixed0 && residual) ? 0 : b.backend[o00 + k];
+#pragma unroll
+      for (int i = 0; i < 8; i++) cnt[i] += (be == i);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) G = cnt[i] > G ? cnt[i] : G;
+  } else if (nbc) G = 1;
+  int K0p = k0_class(K0r);
+  bool fast = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22));
+  if (nbc) {
+    // allowed group sizes per class: nbc*G in {2,4,6,8,12,16}
+    int Gp = 0;
+    if (nbc == 2) Gp = G <= 4 ? (G < 1 ? 1 : G) : (G <= 6 ? 6 : (G <= 8 ? 8 : 0));
+    else if (nbc == 3) Gp = G <= 2 ? 2 : (G <= 4 ? 4 : 0);
+    else if (nbc == 4) Gp = G <= 2 ? (G < 1 ? 1 : G) : (G <= 4 ? 4 : 0);
+    else Gp = G <= 1 ? 1 : (G <= 2 ? 2 : 0);
+    if (Gp == 0) fast = false; else if (fast) { G = Gp; K0p = nbc * Gp; }
+  }
+  int width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
   int optbase = width;   // inclusive scan over lanes -> exclusive
 #pragma unroll
   for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
-  const int nslots = __shfl_sync(0xffffffffu, optbase, 31);
+  int nslots = __shfl_sync(0xffffffffu, optbase, 31);
   optbase -= width;
-  const int nslots_pad = (nslots + 3) & ~3;
+  int nslots_pad = (nslots + 3) & ~3;
+  int blob_words = kHdrWords + nslots_pad * (Lp + 5) + (nbc ? 128 : 0);
+  if (fast && (blob_words > kFastBlobWords || (size_t)blob_words > blob_stride)) {
+    // tables too large for the fp32 scorer's window: fall back to the wide class (recompute the plain layout)
+    fast = false;
+    K0p = k0_class(K0r);
+    width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
+    optbase = width;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
+    nslots = __shfl_sync(0xffffffffu, optbase, 31);
+    optbase -= width;
+    nslots_pad = (nslots + 3) & ~3;
+  }
   unsigned long long outer = (lane >= 2 && lane < Np) ? (unsigned long long)Kp : 1ull;
   unsigned long long base = fixed ? (unsigned long long)fk * mystride : 0ull;
 #pragma unroll
   for (int off = 16; off; off >>= 1) { outer *= __shfl_xor_sync(0xffffffffu, outer, off); base += __shfl_xor_sync(0xffffffffu, base, off); }
-  const uint32_t deps0 = __shfl_sync(0xffffffffu, deps, 0);
+  const uint32_t deps0 = __shfl_sync(0xffffffffu, deps, 0), deps1 = __shfl_sync(0xffffffffu, deps, 1);
 
   if (lane == 0) {
     h->status = DYPLAN_ST_OK; h->n_int = Np; h->n_orig = N; h->orient = orient; h->K0 = K0r; h->K1 = K1r; h->K0p = K0p;
     h->slo = b.slo_us[r]; h->nslots_pad = nslots_pad; h->n0 = n0; h->conn01 = (deps0 >> 1) & 1;
     h->skip_mask = residual ? fmask : 0u; h->outer_total = outer; h->base_idx = base;
     for (int bb = 0; bb < 8; bb++) h->cap[bb] = (b.cap && bb < B) ? b.cap[r * B + bb] : INT32_MAX;
+    h->klass = fast ? kClassFast : kClassWide; h->nbc = fast ? nbc : 0; h->Lp = Lp;
+    const long long slo = b.slo_us[r];
+    h->slo_f = (float)(slo < sum_lat ? slo : sum_lat);
+    h->S01 = ((deps0 >> 1) & 1) ? 1.0f : kBigF;
+    h->big12 = ((deps1 >> 2) & 1) ? 0.0f : kBigF;
+    h->big02 = ((deps0 >> 2) & 1) ? 0.0f : kBigF;
+    h->blob_words = fast ? blob_words : 0;
+    for (int bb = 0; bb < 8; bb++) {
+      long long c = (b.cap && bb < B) ? (long long)b.cap[r * B + bb] : sum_dem;
+      h->capf[bb] = (float)(c < sum_dem ? c : sum_dem);
+    }
   }
   if (lane < 16) {
     h->Kp[lane] = lane < Np ? Kp : 1;
     h->deps[lane] = lane < Np ? deps : 0;
     h->optbase[lane] = lane < Np ? optbase : 0;
-    h->fixk[lane] = fixed ? fk : -1;
     h->stride[lane] = (lane < Np && !fixed) ? mystride : 0ull;
   }
 
-  // ---- tables: dem0b [16][8], lat [slot][L], f [slot], dem [slot], be [slot] ----
+  // ---- tables.  wide: dem0b [16][8], lat [slot][L] (int32), f [slot], dem [slot], be [slot]
+  //              fast: nlat [slot][Lp] (fp32, negated), f [slot], dem [slot] (fp32), be [slot], idxc [slot] (u64),
+  //                    dem1b [16][8] (fp32, caps only); node 0's slots are grouped by backend when caps exist ----
   int* t_dem0b = (int*)(blob + kHdrWords);
   int* t_lat = t_dem0b + kDem0bWords;
   float* t_f = (float*)(t_lat + nslots_pad * L);
   int* t_dem = (int*)(t_f + nslots_pad);
   int* t_be = t_dem + nslots_pad;
-  for (int i = lane; i < kDem0bWords; i += 32) t_dem0b[i] = 0;
+  float* q_nlat = (float*)(blob + kHdrWords);
+  float* q_f = q_nlat + nslots_pad * Lp;
+  float* q_dem = q_f + nslots_pad;
+  int* q_be = (int*)(q_dem + nslots_pad);
+  unsigned long long* q_idxc = (unsigned long long*)(q_be + nslots_pad);
+  float* q_dem1b = (float*)(q_idxc + nslots_pad);
+  if (!fast) for (int i = lane; i < kDem0bWords; i += 32) t_dem0b[i] = 0;
+  else if (nbc) for (int i = lane; i < 128; i += 32) q_dem1b[i] = 0.0f;
   __syncwarp();
   for (int s0 = 0; s0 < nslots_pad; s0 += 32) {   // uniform trip count: the body shuffles
     const int s = s0 + lane;
@@ -206,16 +273,31 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       if (s >= ob && s < ob + w) { node = i; k = s - ob; }
     }
     int ne = -1, nK = 1, no0 = 0, nfix = 0, nfk = 0;
+    unsigned long long nstride = 0;
     for (int i = 0; i < Np; i++) {
       const int ee = __shfl_sync(0xffffffffu, e, i), kk = __shfl_sync(0xffffffffu, myK, i), oo = __shfl_sync(0xffffffffu, myo0, i);
       const int ff = __shfl_sync(0xffffffffu, (int)fixed, i), fkk = __shfl_sync(0xffffffffu, fk, i);
-      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; }
+      const unsigned long long ss = __shfl_sync(0xffffffffu, mystride, i);
+      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; nstride = ss; }
+    }
+    bool pad = node < 0 || (node == 0 && k >= K0r);
+    if (fast && nbc && node == 0) {
+      // slot k = group g (backend g), position p: the p-th candidate option of node 0 on backend g
+      const int g = k / G, pp = k % G;
+      int found = -1, seen = 0;
+      for (int kk = 0; kk < nK; kk++) {
+        if (nfix && kk != nfk) continue;
+        const int be = (ne < 0 || (nfix && residual)) ? 0 : b.backend[no0 + kk];
+        if (be == g) { if (seen == pp) found = kk; seen++; }
+      }
+      if (ne < 0) found = (g == 0 && pp == 0) ? 0 : -1;   // dummy node: one neutral option
+      pad = found < 0;
+      k = nfix ? 0 : (found < 0 ? 0 : found);           // k = enumerated digit value (0 for a pinned node)
     }
     int dl[DYPLAN_MAX_LEVELS];
 #pragma unroll
     for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = 0;
     float f = 1.0f; int dem = 0, be = 0;
-    const bool pad = node < 0 || (node == 0 && k >= K0r);
     if (pad) {
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = INT32_MAX;
@@ -228,69 +310,109 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) if (l < L) dl[l] = (int)scaled(tau, mult[l * B + be]);
       f = (float)factor64(b.vuln[n0 + ne], b.acc[o]);
     }
-    if (active) {
+    if (active && !fast) {
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) if (l < L) t_lat[s * L + l] = dl[l];
       t_f[s] = f; t_dem[s] = dem; t_be[s] = be;
       if (node == 0 && !pad) t_dem0b[k * 8 + be] = dem;
     }
+    if (active && fast) {
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
+        if (l < Lp) q_nlat[s * Lp + l] = pad ? -2.0f * kBigF : -(float)dl[l < L ? l : 0];   // padded levels repeat level 0 (their threshold never admits a plan)
+      q_f[s] = pad ? 0.0f : f; q_dem[s] = (float)dem; q_be[s] = be;
+      q_idxc[s] = (pad || ne < 0 || nfix) ? 0ull : (unsigned long long)k * nstride;
+      if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = (float)dem;
+    }
   }
 }
 
-// Single block: totals, items per request, exclusive scan.
-__global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
-  __shared__ unsigned long long s_sum[1024];
-  __shared__ unsigned long long s_plans[1024];
-  __shared__ uint32_t s_cnt[1024];
-  const int tid = threadIdx.x;
-  const long long R = a.in.R;
-  const size_t blob_stride = blob_stride_words(a.L);
-  const long long chunk = (R + 1023) / 1024;
-  const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
-  unsigned long long so = 0, sp = 0;
-  for (long long r = r0; r < r1; r++) {
-    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
-    if (h->status == DYPLAN_ST_OK) { so += h->outer_total; sp += h->outer_total * (unsigned long long)(h->K0 * h->K1); }
-  }
-  s_sum[tid] = so; s_plans[tid] = sp;
-  __syncthreads();
-  for (int off = 512; off; off >>= 1) { if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_plans[tid] += s_plans[tid + off]; } __syncthreads(); }
-  const unsigned long long total_outer = s_sum[0], total_plans = s_plans[0];
-  __syncthreads();
-  // outer indices per work item: a multiple of the block size; ~16K items when there is enough work,
-  // never more than max_items - R extra items.
-  const unsigned long long target = 16384;
-  unsigned long long pio = (total_outer + target - 1) / target;
-  const unsigned long long extra = a.max_items > (unsigned long long)R ? a.max_items - (unsigned long long)R : 1;
-  const unsigned long long need = (total_outer + extra - 1) / extra;
-  if (need > pio) pio = need;
-  pio = ((pio + kBlock - 1) / kBlock) * kBlock;
-  if (pio < (unsigned long long)kBlock) pio = kBlock;
-  uint32_t cnt = 0;
-  for (long long r = r0; r < r1; r++) {
-    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
-    if (h->status == DYPLAN_ST_OK) cnt += (uint32_t)((h->outer_total + pio - 1) / pio);
-  }
+// Single block: totals, work items per request and scorer class, exclusive scans.
+// Wide class: an item is a range of outer indices handled by one block of k_score.  Fast class: an item is a range
+// of outer indices handled by one warp of k_fscore.  Partial records of fast items follow those of the wide items.
+__device__ __forceinline__ uint32_t block_exclusive_scan_1024(uint32_t* s_cnt, int tid, uint32_t cnt) {
   s_cnt[tid] = cnt;
   __syncthreads();
-  // inclusive scan (Hillis-Steele over 1024 entries)
-  for (int off = 1; off < 1024; off <<= 1) {
+  for (int off = 1; off < 1024; off <<= 1) {   // Hillis-Steele over 1024 entries
     uint32_t v = tid >= off ? s_cnt[tid - off] : 0;
     __syncthreads();
     s_cnt[tid] += v;
     __syncthreads();
   }
-  uint32_t run = s_cnt[tid] - cnt;
+  return s_cnt[tid] - cnt;
+}
+
+__global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
+  __shared__ unsigned long long s_sum[1024];
+  __shared__ unsigned long long s_sumf[1024];
+  __shared__ unsigned long long s_plans[1024];
+  __shared__ uint32_t s_cnt[1024];
+  __shared__ uint32_t s_nf[1024];
+  const int tid = threadIdx.x;
+  const long long R = a.in.R;
+  const size_t blob_stride = blob_stride_words(a.L);
+  const long long chunk = (R + 1023) / 1024;
+  const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
+  unsigned long long so = 0, sf = 0, sp = 0;
+  uint32_t nf = 0;
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
-    a.item_off[r] = run;
-    if (h->status == DYPLAN_ST_OK) run += (uint32_t)((h->outer_total + pio - 1) / pio);
+    if (h->status == DYPLAN_ST_OK) {
+      if (h->klass == kClassFast) { sf += h->outer_total; nf++; } else so += h->outer_total;
+      sp += h->outer_total * (unsigned long long)(h->K0 * h->K1);
+    }
+  }
+  s_sum[tid] = so; s_sumf[tid] = sf; s_plans[tid] = sp; s_nf[tid] = nf;
+  __syncthreads();
+  for (int off = 512; off; off >>= 1) {
+    if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_sumf[tid] += s_sumf[tid + off]; s_plans[tid] += s_plans[tid + off]; s_nf[tid] += s_nf[tid + off]; }
+    __syncthreads();
+  }
+  const unsigned long long total_w = s_sum[0], total_f = s_sumf[0], total_plans = s_plans[0];
+  const uint32_t n_fast = s_nf[0];
+  __syncthreads();
+  // wide: outer indices per item, a multiple of the block size; ~16K items when there is enough work
+  const unsigned long long budget = a.max_items > (unsigned long long)(2 * R + 2) ? (a.max_items - (unsigned long long)(2 * R + 2)) / 2 : 1;
+  unsigned long long pio = (total_w + 16383) / 16384;
+  unsigned long long need = (total_w + budget - 1) / budget;
+  if (need > pio) pio = need;
+  pio = ((pio + kBlock - 1) / kBlock) * kBlock;
+  if (pio < (unsigned long long)kBlock) pio = kBlock;
+  // fast: outer indices per item, a multiple of the warp size; target_items_f items when there is enough work
+  const unsigned long long tgt = a.target_items_f ? a.target_items_f : 1;
+  unsigned long long pif = (total_f + tgt - 1) / tgt;
+  need = (total_f + budget - 1) / budget;
+  if (need > pif) pif = need;
+  pif = ((pif + 31) / 32) * 32;
+  if (pif < 32) pif = 32;
+  uint32_t cw = 0, cf = 0;
+  for (long long r = r0; r < r1; r++) {
+    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+    if (h->status != DYPLAN_ST_OK) continue;
+    if (h->klass == kClassFast) cf += (uint32_t)((h->outer_total + pif - 1) / pif);
+    else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
+  }
+  uint32_t runw = block_exclusive_scan_1024(s_cnt, tid, cw);
+  const uint32_t total_items_w = s_cnt[1023];
+  __syncthreads();
+  uint32_t runf = block_exclusive_scan_1024(s_cnt, tid, cf);
+  const uint32_t total_items_f = s_cnt[1023];
+  for (long long r = r0; r < r1; r++) {
+    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+    a.item_off[r] = runw;
+    a.item_off_f[r] = runf;
+    if (h->status != DYPLAN_ST_OK) continue;
+    if (h->klass == kClassFast) runf += (uint32_t)((h->outer_total + pif - 1) / pif);
+    else runw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
   if (tid == 1023) {
-    a.item_off[R] = s_cnt[1023];
+    a.item_off[R] = total_items_w;
+    a.item_off_f[R] = total_items_f;
     CallState* st = a.st;
-    st->total_outer = total_outer; st->total_plans = total_plans; st->per_item_outer = pio; st->slow_steps = 0;
-    st->total_items = s_cnt[1023]; st->next_item = 0; st->mult_invalid = 0; st->pad = 0;
+    st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
+    st->slow_steps = 0;
+    st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
+    st->fast_requests = n_fast; st->pad = 0;
   }
 }
 
