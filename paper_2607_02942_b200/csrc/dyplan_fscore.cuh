@@ -21,24 +21,35 @@ namespace dyplan {
 template <int L>
 struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
-  Best best[L * 32];               // [level][lane]: the lane's incumbent (touched by the slow path only)
+  Best best[8];                    // the warp's incumbent per level (written by the cooperative slow path only)
   int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
+  float scr[40];                   // slow path: the flagged lane's group state, broadcast through shared memory
   unsigned long long bar;          // mbarrier of the TMA copy
   unsigned long long pad;
 };
 
-// Loop nest of one lane over its range of outer indices (digits of internal nodes >= 2, odometer order):
-//   heavy step  (a digit >= 3 changed)  slack DP of nodes top..3 over local-memory arrays, node-2 context, thresholds
-//                                       refreshed from what every warp published in g_thr
-//   light step  (digit 2)               u2, running minimum, inputs of the middle loop, C2, cap slack
+// scratch layout of the cooperative slow path
+constexpr int kScrC1 = 0, kScrS1 = 1, kScrAp1 = 9, kScrU1 = 17, kScrR2 = 25, kScrIdx = 34;
+
+// Loop nest of one lane over `steps` outer indices (digits of internal nodes >= 2, odometer order).  Every lane of
+// the warp runs the same number of steps (a lane whose own range is shorter keeps walking with C = 0, which can
+// never produce a candidate), so the warp stays converged and the slow path can be cooperative:
+//   heavy step  (a digit >= 3 changed)  slack DP of nodes top..3 over local-memory arrays, node-2 context
+//   light step  (digit 2)               u2, running minimum, inputs of the middle loop, C2, cap slack; thresholds
+//                                       refreshed from what every warp of the request published in g_thr
 //   middle loop (digit 1)               ap1_l = min(A0q1_l, (U1_l + 1 - d1_l) * S01): slack bound (+1) of node 0
 //   inner block (digit 0, unrolled)     the screen; tables in registers
-//   slow path                           exact re-walk of the K0P-wide group
+//   slow path   (any lane saw z > 0)    for each flagged lane: its group state goes to shared memory, the 32 lanes
+//                                       re-evaluate the K0P x L (plan, level) pairs one per lane with the exact
+//                                       order 7 (T and the canonical index), candidates update the warp's incumbent
 template <int L, int K0P, int NB>
-__device__ __noinline__ void frange(const uint32_t* __restrict__ sb, unsigned long long o_begin, unsigned long long o_count,
-                                    int* w_thr, Best* my_best, int* g_thr, const int Lr, unsigned* __restrict__ slow_io) {
+__device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned long long o_begin, unsigned long long my_count,
+                                    unsigned long long steps, int* g_thr, const int Lr, unsigned* __restrict__ slow_io) {
   constexpr int NBX = NB ? NB : 1;
   constexpr int G = NB ? K0P / NB : K0P;
+  const int lane = threadIdx.x & 31;
+  const uint32_t* sb = ws->blob;
+  int* w_thr = ws->thr;
   unsigned slow_steps = 0;
   const ReqHdr* h = (const ReqHdr*)sb;
   const int nsp = h->nslots_pad;
@@ -87,10 +98,16 @@ __device__ __noinline__ void frange(const uint32_t* __restrict__ sb, unsigned lo
   }
   int k2 = dig[2];
   int top = Np - 1;   // recompute nodes top..3
+  bool need_heavy = true;
   float X2[L], Rm3[L], U1r[L], A0r[L], D3[NBX];
-  float C3;
+  float C3 = 0.0f;
   float nthrm[L];   // -pred(thr_l): the screen's addend
-  for (;;) {
+  // lane l < Lr reads the bits of the best C the request's warps have published for level l, one light step ahead
+  const int* gaddr = g_thr + (lane < Lr ? lane : 0);
+  int gpub = 0;
+  for (unsigned long long step = 0; step < steps; step++) {
+    if (need_heavy) {
+    need_heavy = false;
     // ---- heavy step ----
     for (int i = top; i >= 3; --i) {
       const int slot = h->optbase[i] + dig[i];
@@ -136,121 +153,166 @@ __device__ __noinline__ void frange(const uint32_t* __restrict__ sb, unsigned lo
     C3 = Cp[3];
 #pragma unroll
     for (int b = 0; b < NBX; b++) D3[b] = Dp[3][b];
-    // thresholds: take what the other warps of this request have published meanwhile
-#pragma unroll
-    for (int l = 0; l < L; l++) {
-      const int g = l < Lr ? __ldcg(&g_thr[l]) : 0;
-      int t = ((volatile int*)w_thr)[l];
-      if (g > t) { atomicMax(&w_thr[l], g); t = g; }
-      nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
     }
-
-    for (;;) {
-      // ---- light step: node 2 takes option k2 ----
-      const int slot2 = ob2 + k2;
-      float R2[L], U1pS[L], A0q1[L];
+    __syncwarp();   // lanes whose heavy step was shorter wait here: the code below runs converged
+    {
+      // thresholds: this warp's, raised by what the other warps of the request had published one light step ago
+      // (the load issued here is consumed at the next step, which keeps its L2 latency off the critical path)
 #pragma unroll
       for (int l = 0; l < L; l++) {
-        const float u2 = X2[l] + s_nlat[slot2 * L + l];
-        R2[l] = fminf(Rm3[l], u2);
-        const float U1 = fminf(U1r[l], u2 + big12);
-        const float a0 = fminf(A0r[l], u2 + big02);
-        A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
-        U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
+        const int t = max(((volatile int*)w_thr)[l], __shfl_sync(0xffffffffu, gpub, l));
+        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
       }
-      const float C2 = C3 * s_f[slot2];
-      float sD2[NBX];   // cap slack + 1 before nodes 1 and 0
-      if (NB) {
-        const int be2 = s_be[slot2];
-        const float dm2 = s_dem[slot2];
-#pragma unroll
-        for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
-      }
+      gpub = __ldcg(gaddr);
+    }
 
-      for (int k1 = 0; k1 < K1; k1++) {
-        const int slot1 = K0P + k1;
-        float C1 = C2 * s_f[slot1];
-        float s1[NBX];
-        if (NB) {
-          float smin = kBigF;
+    // ---- light step: node 2 takes option k2 ----
+    const bool live = step < my_count;
+    const int slot2 = ob2 + k2;
+    float R2[L], U1pS[L], A0q1[L];
 #pragma unroll
-          for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - s_dem1b[k1 * 8 + b]; smin = fminf(smin, s1[b]); }
-          C1 *= __saturatef(smin);   // a backend is already over its cap: no plan of this group can be a candidate
-        }
-        float ap1[L];
+    for (int l = 0; l < L; l++) {
+      const float u2 = X2[l] + s_nlat[slot2 * L + l];
+      R2[l] = fminf(Rm3[l], u2);
+      const float U1 = fminf(U1r[l], u2 + big12);
+      const float a0 = fminf(A0r[l], u2 + big02);
+      A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
+      U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
+    }
+    const float C2 = live ? C3 * s_f[slot2] : 0.0f;   // a lane past its own range scores nothing
+    float sD2[NBX];   // cap slack + 1 before nodes 1 and 0
+    if (NB) {
+      const int be2 = s_be[slot2];
+      const float dm2 = s_dem[slot2];
 #pragma unroll
-        for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
-        // ---- screen: K0P x L evaluations ----
-        float zm = 0.0f;
+      for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
+    }
+
+    for (int k1 = 0; k1 < K1; k1++) {
+      const int slot1 = K0P + k1;
+      float C1 = C2 * s_f[slot1];
+      float s1[NBX];
+      if (NB) {
+        float smin = kBigF;
 #pragma unroll
-        for (int k0 = 0; k0 < K0P; k0++) {
-          float P = C1 * f0[k0];
-          if (NB) P *= __saturatef(s1[k0 / G] + ndem0[k0]);
-          float z[L];
+        for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - s_dem1b[k1 * 8 + b]; smin = fminf(smin, s1[b]); }
+        C1 *= __saturatef(smin);   // a backend is already over its cap: no plan of this group can be a candidate
+      }
+      float ap1[L];
 #pragma unroll
-          for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, nthrm[l]);
+      for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
+      // ---- screen: K0P x L evaluations ----
+      float zm = 0.0f;
 #pragma unroll
-          for (int l = 0; l + 1 < L; l += 2) zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
-          if (L & 1) zm = fmaxf(zm, z[L - 1]);
-        }
-        if (__builtin_expect(zm > 0.0f, 0)) {
-          // ---- slow path: exact order on this group ----
-          slow_steps++;
-          unsigned long long idx1 = h->base_idx + s_idxc[slot1] + s_idxc[slot2];
-          for (int i = 3; i < Np; i++) idx1 += s_idxc[h->optbase[i] + dig[i]];
+      for (int k0 = 0; k0 < K0P; k0++) {
+        float P = C1 * f0[k0];
+        if (NB) P *= __saturatef(s1[k0 / G] + ndem0[k0]);
+        float z[L];
 #pragma unroll
-          for (int g = 0; g < NBX; g++) {
-            for (int p = 0; p < G; p++) {
-              const int k0 = g * G + p;
-              float P = __fmul_rn(C1, s_f[k0]);
-              if (NB) P = __fmul_rn(P, __saturatef(s1[g] - s_dem[k0]));
-              if (!(P > 0.0f)) continue;
-              const unsigned long long idx = idx1 + s_idxc[k0];
+        for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, nthrm[l]);
 #pragma unroll
-              for (int l = 0; l < L; l++) {
-                const float t1 = ap1[l] + s_nlat[k0 * L + l];   // slack + 1 of node 0's path
-                if (!(t1 >= 1.0f)) continue;
-                const int tb = ((volatile int*)w_thr)[l];
-                if (P < __int_as_float(tb)) continue;
-                const float u1p = fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]) * rS01;   // slack + 1 of node 1
-                const float ms1 = fminf(fminf(t1, u1p), R2[l] + 1.0f);                  // least slack + 1
-                const int T = (int)((slo + 1.0f) - ms1);
-                Best* bp = &my_best[l * 32];
-                const Best cur = *bp;
-                if (better(P, T, idx, cur)) {
-                  Best nb; nb.C = P; nb.T = T; nb.idx = idx;
-                  *bp = nb;
-                  const int cb = __float_as_int(P);
-                  if (cb > tb) { atomicMax(&w_thr[l], cb); if (l < Lr) atomicMax(&g_thr[l], cb); }
+        for (int l = 0; l + 1 < L; l += 2) zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
+        if (L & 1) zm = fmaxf(zm, z[L - 1]);
+      }
+      unsigned flagged = __ballot_sync(0xffffffffu, zm > 0.0f);
+      if (__builtin_expect(flagged != 0u, 0)) {
+        // ---- cooperative slow path: exact order on the group of every flagged lane ----
+        while (flagged) {
+          const int src = __ffs(flagged) - 1;
+          flagged &= flagged - 1;
+          {
+            // first take what the other warps have published by now: most flags are stale-threshold flags
+            const int pub = __ldcg(gaddr);
+            if (lane < Lr && pub > ((volatile int*)w_thr)[lane]) w_thr[lane] = pub;
+          }
+          if (lane == src) {
+            slow_steps++;
+            ws->scr[kScrC1] = C1;
+#pragma unroll
+            for (int b = 0; b < NBX; b++) ws->scr[kScrS1 + b] = NB ? s1[b] : 0.0f;
+#pragma unroll
+            for (int l = 0; l < L; l++) { ws->scr[kScrAp1 + l] = ap1[l]; ws->scr[kScrU1 + l] = U1pS[l]; ws->scr[kScrR2 + l] = R2[l]; }
+          }
+          __syncwarp();
+          const float gC1 = ws->scr[kScrC1];
+          bool have_idx = false;
+          unsigned long long gidx1 = 0;
+          for (int e0 = 0; e0 < K0P * L; e0 += 32) {
+            const int e = e0 + lane;
+            bool cand = false;
+            float P = 0.0f;
+            int T = 0, l = 0, k0 = 0;
+            if (e < K0P * L) {
+              k0 = e / L;
+              l = e - k0 * L;
+              P = __fmul_rn(gC1, s_f[k0]);
+              if (NB) P = __fmul_rn(P, __saturatef(ws->scr[kScrS1 + k0 / G] - s_dem[k0]));
+              const float t1 = ws->scr[kScrAp1 + l] + s_nlat[e];          // slack + 1 of node 0's path
+              const float u1p = fmaf(s_nlat[slot1 * L + l], S01, ws->scr[kScrU1 + l]) * rS01;   // slack + 1 of node 1
+              const float ms1 = fminf(fminf(t1, u1p), ws->scr[kScrR2 + l] + 1.0f);              // least slack + 1
+              T = (int)((slo + 1.0f) - ms1);
+              // phase 1: feasible, and not worse than the warp's incumbent on (C desc, T asc)
+              const float bC = ((volatile float*)&ws->best[l].C)[0];
+              const int bT = ((volatile int*)&ws->best[l].T)[0];
+              cand = P > 0.0f && t1 >= 1.0f && (P > bC || (P == bC && T <= bT)) && P >= __int_as_float(((volatile int*)w_thr)[l]);
+            }
+            unsigned cm = __ballot_sync(0xffffffffu, cand);
+            if (cm && !have_idx) {
+              // phase 2 needs the canonical index of the flagged lane's prefix
+              have_idx = true;
+              if (lane == src) {
+                unsigned long long idx1 = h->base_idx + s_idxc[slot1] + s_idxc[slot2];
+                for (int i = 3; i < Np; i++) idx1 += s_idxc[h->optbase[i] + dig[i]];
+                *(unsigned long long*)&ws->scr[kScrIdx] = idx1;
+              }
+              __syncwarp();
+              gidx1 = *(const unsigned long long*)&ws->scr[kScrIdx];
+            }
+            const unsigned long long idx = gidx1 + s_idxc[k0];
+            while (cm) {
+              const int c = __ffs(cm) - 1;
+              cm &= cm - 1;
+              const int cl = __shfl_sync(0xffffffffu, l, c);
+              const float cP = __shfl_sync(0xffffffffu, P, c);
+              const int cT = __shfl_sync(0xffffffffu, T, c);
+              const unsigned long long cidx = __shfl_sync(0xffffffffu, idx, c);
+              Best cur;
+              cur.C = ((volatile float*)&ws->best[cl].C)[0]; cur.T = ((volatile int*)&ws->best[cl].T)[0];
+              cur.idx = ((volatile unsigned long long*)&ws->best[cl].idx)[0];
+              if (better(cP, cT, cidx, cur)) {   // warp-uniform
+                __syncwarp();
+                if (lane == 0) {
+                  Best nb; nb.C = cP; nb.T = cT; nb.idx = cidx;
+                  ws->best[cl] = nb;
+                  const int cb = __float_as_int(cP);
+                  if (cb > w_thr[cl]) { w_thr[cl] = cb; if (cl < Lr) atomicMax(&g_thr[cl], cb); }
                 }
+                __syncwarp();
               }
             }
           }
+          __syncwarp();
+        }
 #pragma unroll
-          for (int l = 0; l < L; l++) {
-            const int t = ((volatile int*)w_thr)[l];
-            nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
-          }
+        for (int l = 0; l < L; l++) {
+          const int t = ((volatile int*)w_thr)[l];
+          nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
         }
       }
-      // ---- advance ----
-      if (--o_count == 0) goto done;
-      if (++k2 < K2) continue;
-      k2 = 0;
-      break;
     }
-    {
+    // ---- advance ----
+    if (++k2 >= K2) {
+      k2 = 0;
       int i = 3;
-      for (;;) {
+      for (; i < Np; i++) {
         const int d = dig[i] + 1;
         if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
         dig[i] = 0;
-        i++;
       }
-      top = i;
+      top = i < Np ? i : Np - 1;   // ran off the request's last outer index (only a lane past its own range does)
+      need_heavy = true;
     }
   }
-done:
   *slow_io += slow_steps;
 }
 
@@ -296,22 +358,24 @@ __global__ void __launch_bounds__(kFastWarps * 32, 4) k_fscore(const CallArgs a)
     const ReqHdr* h = (const ReqHdr*)ws->blob;
     int* g_thr = (int*)a.gthr + r * Lr;
     if (lane < 8) ws->thr[lane] = lane < Lr ? __ldcg(&g_thr[lane]) : 0x40000000;   // padded levels: 2.0f, never admitted
-#pragma unroll
-    for (int l = 0; l < L; l++) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; ws->best[l * 32 + lane] = e; }
+    if (lane < 8) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; ws->best[lane] = e; }
     __syncwarp();
     const uint32_t first_item = __ldg(&a.item_off_f[r]);
-    const unsigned long long ob = (unsigned long long)(item - first_item) * pif;
-    const unsigned long long oe = min(ob + pif, (unsigned long long)h->outer_total);
+    const unsigned long long pir = fast_item_outer(pif, h->Kp[2]);
+    const unsigned long long ob = (unsigned long long)(item - first_item) * pir;
+    const unsigned long long oe = min(ob + pir, (unsigned long long)h->outer_total);
     const unsigned long long len = oe - ob;
-    const unsigned long long per = (len + 31) / 32;
+    // lanes take consecutive sub-ranges of the same length (a multiple of node 2's radix, so that every lane is at
+    // the same k2 and the heavy steps coincide); every lane runs `per` steps, the ones past its range score nothing
+    const unsigned long long K2u = (unsigned long long)h->Kp[2];
+    const unsigned long long per = (((len + 31) / 32 + K2u - 1) / K2u) * K2u;
     const unsigned long long tb = min(ob + (unsigned long long)lane * per, oe);
     const unsigned long long te = min(tb + per, oe);
-
-    if (te > tb) {
+    {
       const unsigned long long n = te - tb;
-      Best* mb = ws->best + lane;
+      const unsigned long long t0 = n ? tb : 0ull;   // an idle lane walks from outer index 0 (with C = 0)
       switch (h->nbc * 32 + h->K0p) {
-#define DYPLAN_FCASE(NB_, K_) case NB_ * 32 + K_: frange<L, K_, NB_>(ws->blob, tb, n, ws->thr, mb, g_thr, Lr, &slow_steps); break;
+#define DYPLAN_FCASE(NB_, K_) case NB_ * 32 + K_: frange<L, K_, NB_>(ws, t0, n, per, g_thr, Lr, &slow_steps); break;
         DYPLAN_FCASE(0, 2) DYPLAN_FCASE(0, 4) DYPLAN_FCASE(0, 6) DYPLAN_FCASE(0, 8) DYPLAN_FCASE(0, 12) DYPLAN_FCASE(0, 16)
         DYPLAN_FCASE(2, 2) DYPLAN_FCASE(2, 4) DYPLAN_FCASE(2, 6) DYPLAN_FCASE(2, 8) DYPLAN_FCASE(2, 12) DYPLAN_FCASE(2, 16)
         DYPLAN_FCASE(3, 6) DYPLAN_FCASE(3, 12)
@@ -322,13 +386,9 @@ __global__ void __launch_bounds__(kFastWarps * 32, 4) k_fscore(const CallArgs a)
       }
     }
     __syncwarp();
-    // ---- warp arg-best per level (shuffles); lane l keeps level l ----
+    // ---- the warp's incumbents are the item's records; lane l keeps level l ----
     Best mine; mine.C = -1.0f; mine.T = INT32_MAX; mine.idx = kNoIdx;
-#pragma unroll
-    for (int l = 0; l < L; l++) {
-      const Best v = warp_best(ws->best[l * 32 + lane]);
-      if (lane == l) mine = v;
-    }
+    if (lane < Lr) mine = ws->best[lane];
     if (lane < Lr) {
       Partial p; p.C = mine.C; p.T = mine.T; p.idx = mine.idx;
       a.partial[(size_t)(rec_base + item) * Lr + lane] = p;

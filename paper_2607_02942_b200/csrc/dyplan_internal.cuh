@@ -23,6 +23,12 @@ constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): every latency 
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
 constexpr float kBigF = 16777216.0f; // 2^24
+// fast class: outer indices per work item of a request whose node 2 has K2 options -- the call-wide figure rounded up
+// so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)
+__host__ __device__ inline unsigned long long fast_item_outer(unsigned long long pif, int K2) {
+  const unsigned long long q = 32ull * (unsigned long long)(K2 < 1 ? 1 : K2);
+  return ((pif + q - 1) / q) * q;
+}
 __host__ __device__ inline int level_class(int L) { return L <= 4 ? L : (L <= 6 ? 6 : 8); }
 
 // Per-request staged problem in "internal" node order.  Internal node 0 is the innermost

@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     if (h->status != DYPLAN_ST_OK) continue;
-    if (h->klass == kClassFast) cf += (uint32_t)((h->outer_total + pif - 1) / pif);
+    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2]); cf += (uint32_t)((h->outer_total + q - 1) / q); }
     else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
   uint32_t runw = block_exclusive_scan_1024(s_cnt, tid, cw);
@@ -402,7 +402,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     a.item_off[r] = runw;
     a.item_off_f[r] = runf;
     if (h->status != DYPLAN_ST_OK) continue;
-    if (h->klass == kClassFast) runf += (uint32_t)((h->outer_total + pif - 1) / pif);
+    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2]); runf += (uint32_t)((h->outer_total + q - 1) / q); }
     else runw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
   if (tid == 1023) {
