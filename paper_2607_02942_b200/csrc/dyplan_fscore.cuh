@@ -104,6 +104,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
   float nthrm[L];   // -pred(thr_l): the screen's addend
   // lane l < Lr reads the bits of the best C the request's warps have published for level l, one light step ahead
   const int* gaddr = g_thr + (lane < Lr ? lane : 0);
+  asm volatile("" : "+l"(gaddr));   // keep the address in its own register pair (not rematerialised into a scratch pair)
   int gpub = 0;
   for (unsigned long long step = 0; step < steps; step++) {
     if (need_heavy) {
@@ -188,6 +189,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
     }
 
+#pragma unroll 2
     for (int k1 = 0; k1 < K1; k1++) {
       const int slot1 = K0P + k1;
       float C1 = C2 * s_f[slot1];
@@ -217,14 +219,12 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       unsigned flagged = __ballot_sync(0xffffffffu, zm > 0.0f);
       if (__builtin_expect(flagged != 0u, 0)) {
         // ---- cooperative slow path: exact order on the group of every flagged lane ----
+        // (what the other warps have published by now is fetched meanwhile and applied on the way out: many flags
+        // are stale-threshold flags, and the next groups should not raise them again)
+        const int pub = __ldcg(gaddr);
         while (flagged) {
           const int src = __ffs(flagged) - 1;
           flagged &= flagged - 1;
-          {
-            // first take what the other warps have published by now: most flags are stale-threshold flags
-            const int pub = __ldcg(gaddr);
-            if (lane < Lr && pub > ((volatile int*)w_thr)[lane]) w_thr[lane] = pub;
-          }
           if (lane == src) {
             slow_steps++;
             ws->scr[kScrC1] = C1;
@@ -293,6 +293,8 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
           }
           __syncwarp();
         }
+        if (lane < Lr && pub > ((volatile int*)w_thr)[lane]) w_thr[lane] = pub;
+        __syncwarp();
 #pragma unroll
         for (int l = 0; l < L; l++) {
           const int t = ((volatile int*)w_thr)[l];
@@ -317,7 +319,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 }
 
 template <int L>
-__global__ void __launch_bounds__(kFastWarps * 32, 4) k_fscore(const CallArgs a) {
+__global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(const CallArgs a) {
   __shared__ FWarpShared<L> s_w[kFastWarps];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   FWarpShared<L>* ws = &s_w[wid];

@@ -325,6 +325,50 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = (float)dem;
     }
   }
+
+  // ---- seed the incumbent thresholds of a fast-class request: score a few hundred random plans the
+  // same way k_fscore does (fp32 slack DP, C32 as the product in internal node order from the last node down) and
+  // publish the best feasible C per level.  A threshold is only ever the C32 of a plan that exists and is feasible,
+  // so the enumeration still meets that plan (ties pass the screen) and the result does not depend on the seeds. ----
+  if (fast) {
+    __syncwarp();
+    constexpr int kSeedsPerLane = 16;
+    const float slo_f = h->slo_f;
+    float su[16][DYPLAN_MAX_LEVELS];
+    for (int sidx = 0; sidx < kSeedsPerLane; sidx++) {
+      uint32_t x = (uint32_t)r * 0x9E3779B9u + (uint32_t)(sidx * 32 + lane) * 0x85EBCA6Bu + 0x27D4EB2Fu;
+      float C = 1.0f, D[8], ms[DYPLAN_MAX_LEVELS];
+#pragma unroll
+      for (int i = 0; i < 8; i++) D[i] = 0.0f;
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) ms[l] = slo_f;
+      for (int i = Np - 1; i >= 0; --i) {
+        x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;   // integer hash, one draw per node
+        const int kp = i == 0 ? K0p : h->Kp[i];
+        const int slot = h->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
+        C *= q_f[slot];
+        D[q_be[slot] & 7] += q_dem[slot];
+        const uint32_t dm0 = h->deps[i];
+#pragma unroll
+        for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+          if (l < L) {
+            float m = slo_f;
+            for (uint32_t dm = dm0; dm; dm &= dm - 1) m = fminf(m, su[__ffs(dm) - 1][l]);
+            const float v = m + q_nlat[slot * Lp + l];
+            su[i][l] = v;
+            ms[l] = fminf(ms[l], v);
+          }
+        }
+      }
+      bool capok = C > 0.0f;   // a padding slot of node 0 has f = 0
+      if (nbc) for (int bb = 0; bb < B; bb++) capok &= D[bb] <= h->capf[bb];
+      if (capok) {
+#pragma unroll
+        for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
+          if (l < L && ms[l] >= 0.0f) atomicMax((int*)&a.gthr[r * L + l], __float_as_int(C));
+      }
+    }
+  }
 }
 
 // Single block: totals, work items per request and scorer class, exclusive scans.
