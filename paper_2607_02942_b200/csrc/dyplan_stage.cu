@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   // ---- shape checks, in the oracle's order (load_req, validate, dispatched set, size of the free space) ----
   int st = DYPLAN_ST_OK;
   long long sum_lat = 0, sum_dem = 0;   // largest possible T over the levels / largest possible total demand
+  double min_c = 1.0;                   // smallest possible C (product of the per-node minimum factors)
   const int n0 = b.node_off[r], n1 = b.node_off[r + 1];
   const int N = n1 - n0;
   int K[16], o0[16];
@@ -101,6 +102,17 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
         for (int off = 16; off; off >>= 1) mx += __shfl_xor_sync(0xffffffffu, mx, off);
         bad |= mx > (long long)INT32_MAX;
         if (l < L) sum_lat = mx > sum_lat ? mx : sum_lat; else sum_dem = mx;
+      }
+      // smallest possible C: the fp32 scorer needs every plan's C32 to be a positive normal number
+      if (!bad) {
+        double mn = 1.0;
+        if (lane < N) {
+          const float v = b.vuln[n0 + lane];
+          for (int k = 0; k < nodeK; k++) { const double f = factor64(v, b.acc[nodeo0 + k]); mn = f < mn ? f : mn; }
+        }
+#pragma unroll
+        for (int off = 16; off; off >>= 1) mn *= __shfl_xor_sync(0xffffffffu, mn, off);
+        min_c = mn;
       }
     }
     if (bad) st = DYPLAN_ST_INVALID;
@@ -186,7 +198,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     for (int i = 0; i < 8; i++) G = cnt[i] > G ? cnt[i] : G;
   } else if (nbc) G = 1;
   int K0p = k0_class(K0r);
-  bool fast = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22));
+  bool fast = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)) && min_c >= 1e-30;
   if (nbc) {
     // allowed group sizes per class: nbc*G in {2,4,6,8,12,16}
     int Gp = 0;

@@ -163,6 +163,72 @@ def test_duplicate_options_exact_ties(dy, orc):
     g, ref, c = both(dy, orc, w, "ties")
 
 
+# ---- scorer classes: fp32 slack DP for small exact ranges, int32 slack DP for the rest ----------------
+def gpu_run_stats(dy, w):
+    g = gpu_run(dy, w)
+    return g, dy[1].dyplan_last_stats()
+
+
+def test_baseline_configs_take_the_fp32_scorer(dy):
+    for cfg, R in ((0, 1), (1, 2), (2, 8), (3, 16), (4, 1)):
+        w = wl.make_config(cfg, R=R)
+        if cfg == 4:   # keep the run short: the class is decided per request, before any enumeration
+            w.batch.slo_us[:] = 0
+        _, st = gpu_run_stats(dy, w)
+        assert st["fast_requests"] == w.batch.R, (cfg, st)
+
+
+def _scale_latencies(w, rows, factor):
+    b = w.batch
+    for r in rows:
+        a, e = int(b.opt_off[b.node_off[r]]), int(b.opt_off[b.node_off[r + 1]])
+        b.lat_us[a:e] *= factor
+        b.slo_us[r] = int(min(int(b.slo_us[r]) * factor, 2**31 - 1))
+
+
+@pytest.mark.parametrize("seed,L,B,caps", [(91, 2, 2, True), (92, 4, 3, False), (93, 5, 4, True)])
+def test_wide_class_large_latencies(dy, orc, seed, L, B, caps):
+    # latency sums far above 2^22 us: not exact in fp32, so every request goes to the int32 scorer
+    w = wl.random_workload(seed, R=24, nmin=2, nmax=7, kmin=1, kmax=6, B=B, M=3, L=L, caps=caps)
+    _scale_latencies(w, range(w.batch.R), 3000)
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    assert st["fast_requests"] <= 2        # (a one- or two-node request can still fit under 2^22)
+    check_records(orc, w, g, orc.run(w), where=f"wide-class(seed={seed})")
+
+
+def test_mixed_classes_in_one_batch(dy, orc):
+    w = wl.random_workload(94, R=40, nmin=2, nmax=7, kmin=1, kmax=6, B=2, M=3, L=3, caps=True)
+    _scale_latencies(w, range(0, 40, 3), 3000)
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    assert 0 < st["fast_requests"] < w.batch.R
+    check_records(orc, w, g, orc.run(w), where="mixed-classes")
+
+
+def test_zero_factor_requests_go_to_the_int32_scorer(dy, orc):
+    # f = 1 - v (1 - a) = 0 makes C32 = 0 for real plans; the fp32 screen needs C32 > 0, so k_stage routes them away
+    w = wl.random_workload(95, R=16, nmin=2, nmax=5, kmin=2, kmax=5, B=2, M=2, L=2, caps=False, tool_p=0.0)
+    b = w.batch
+    for r in range(0, 16, 2):
+        n = int(b.node_off[r])
+        b.vuln[n] = 1.0
+        b.acc[int(b.opt_off[n]): int(b.opt_off[n + 1])] = 0.0     # every option of that node: every plan has C = 0
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    assert st["fast_requests"] == 8
+    ref = orc.run(w)
+    check_records(orc, w, g, ref, where="zero-factor")
+    assert (g["corr"].reshape(16, 2)[0::2][g["status"].reshape(16, 2)[0::2] == 0] == 0.0).all()
+
+
+@pytest.mark.parametrize("seed,B,kmax", [(96, 2, 16), (97, 3, 12), (98, 4, 16), (99, 8, 16), (100, 6, 9)])
+def test_fast_class_backend_group_layouts(dy, orc, seed, B, kmax):
+    # caps + many options: node 0's slots are grouped by backend (2/3/4/8 groups); shapes that do not fit go wide
+    w = wl.random_workload(seed, R=20, nmin=2, nmax=4, kmin=2, kmax=kmax, B=B, M=3, L=2, caps=True, tool_p=0.0)
+    both(dy, orc, w, f"groups(seed={seed})")
+
+
 # ---- malformed inputs: per-request status, the rest of the batch still compiles ------------------------
 def test_invalid_requests_are_isolated(dy, orc):
     w = wl.random_workload(51, R=12, nmin=3, nmax=6, kmin=2, kmax=5, B=2, M=3, L=2, caps=True, tool_p=0.0)
