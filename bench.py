@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- the dyplan hot path on N B200s of one node (contract: see the task statement / DESIGN.md section 9).
 
-A "step" is one pass of the whole hot path (K_stage -> K_plan -> K_score with the fused final reduce and bundle
-emission) over one batch of synthetic requests: BASELINE.json configs[1] by default (256 requests, 8-node layered
+A "step" is one pass of the whole hot path (K_stage -> K_plan -> K_fscore / K_score with the fused final reduce and
+bundle emission) over one batch of synthetic requests: BASELINE.json configs[1] by default (256 requests, 8-node layered
 DAGs, 8 options per node, 4 pressure levels: 4.29e9 plans, 1.72e10 (plan, level) evaluations).  Requests are
 independent, so with N > 1 every rank compiles its own batch of the same shape (different seed) and no data-path
 collective exists ("scaling": "weak").
@@ -272,7 +272,7 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
                 "api": "dyplan_compile_host" if w.kind == "compile" else "dyplan_replan_host"},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "k_score", "achieved": achieved, "peak": peak, "unit": "Tinst/s",
+        "roofline": {"bound": "alu", "kernel": "k_fscore" if st.get("fast_requests", 0) else "k_score", "achieved": achieved, "peak": peak, "unit": "Tinst/s",
                      "frac": achieved / peak, "traffic": None,
                      "ops_per_eval": aops, "kernel_ms": k_ms / args.steps,
                      "peak_how": f"{sm_count} SMs x 128 lanes x {sm_max:.0f} MHz (B300_MICROARCH.md: 1 warp-inst/clk/SMSP); DESIGN.md section 8"},
