@@ -221,13 +221,14 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
 
 
   CK(launch_stage(a, stream));
+  CK(launch_seed(a, stream));
   CK(launch_plan(a, stream));
   CK(cudaEventRecord(ctx->ev0, stream));
   CK(kFLaunch[L - 1](a, fgrid, stream));      // fp32 scorer: requests of the fast class
   CK(kLaunch[L - 1](a, nbc, grid, stream));   // int32 scorer: the rest (exits at once when it has no work items)
   CK(cudaEventRecord(ctx->ev1, stream));
   ctx->have_events = true;
-  ctx->last_launches = 4;
+  ctx->last_launches = 5;
   return DYPLAN_OK;
 }
 

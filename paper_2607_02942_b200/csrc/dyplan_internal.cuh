@@ -113,6 +113,7 @@ struct CallArgs {                   // passed by value to the kernels
 // launchers (defined in the .cu files)
 cudaError_t launch_stage(const CallArgs& a, cudaStream_t s);
 cudaError_t launch_plan(const CallArgs& a, cudaStream_t s);
+cudaError_t launch_seed(const CallArgs& a, cudaStream_t s);
 typedef cudaError_t (*score_launcher_t)(const CallArgs& a, int nb_class, int grid, cudaStream_t s);
 typedef cudaError_t (*fscore_launcher_t)(const CallArgs& a, int grid, cudaStream_t s);
 cudaError_t launch_score(const CallArgs& a, int grid, cudaStream_t s);

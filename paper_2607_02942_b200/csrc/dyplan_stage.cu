@@ -337,48 +337,69 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = (float)dem;
     }
   }
+}
 
-  // ---- seed the incumbent thresholds of a fast-class request: score a few hundred random plans the
-  // same way k_fscore does (fp32 slack DP, C32 as the product in internal node order from the last node down) and
-  // publish the best feasible C per level.  A threshold is only ever the C32 of a plan that exists and is feasible,
-  // so the enumeration still meets that plan (ties pass the screen) and the result does not depend on the seeds. ----
-  if (fast) {
-    __syncwarp();
-    constexpr int kSeedsPerLane = 16;
-    const float slo_f = h->slo_f;
-    float su[16][DYPLAN_MAX_LEVELS];
-    for (int sidx = 0; sidx < kSeedsPerLane; sidx++) {
-      uint32_t x = (uint32_t)r * 0x9E3779B9u + (uint32_t)(sidx * 32 + lane) * 0x85EBCA6Bu + 0x27D4EB2Fu;
-      float C = 1.0f, D[8], ms[DYPLAN_MAX_LEVELS];
+// ---- K_seed: seed the incumbent thresholds of the fast-class requests.  One block per request: score
+// a few hundred random plans the same way k_fscore does (fp32 slack DP, C32 as the product in internal node order from
+// the last node down) and publish the best feasible C per level.  A threshold is only ever the C32 of a plan that
+// exists and is feasible, so the enumeration still meets that plan (ties pass the screen) and the result does not
+// depend on the seeds. ----
+constexpr int kSeedThreads = 128, kSeedsPerThread = 4;
+__global__ void __launch_bounds__(kSeedThreads) k_seed(CallArgs a) {
+  __shared__ __align__(16) uint32_t sb[kFastBlobWords];
+  const long long r = blockIdx.x;
+  const int L = a.L, B = a.in.B, tid = threadIdx.x;
+  const uint32_t* blob = a.blob + (size_t)r * blob_stride_words(L);
+  const ReqHdr* gh = (const ReqHdr*)blob;
+  if (gh->status != DYPLAN_ST_OK || gh->klass != kClassFast) return;   // block-uniform
+  const int words = gh->blob_words;
+  for (int i = tid; i < words; i += kSeedThreads) sb[i] = blob[i];
+  __syncthreads();
+  const ReqHdr* sh = (const ReqHdr*)sb;
+  const int nsp = sh->nslots_pad, Lp = sh->Lp, Np = sh->n_int, K0p = sh->K0p, nbc = sh->nbc;
+  const float* p_nlat = (const float*)(sb + kHdrWords);
+  const float* p_f = p_nlat + nsp * Lp;
+  const float* p_dem = p_f + nsp;
+  const int* p_be = (const int*)(p_dem + nsp);
+  const float slo_f = sh->slo_f;
+  float su[16][DYPLAN_MAX_LEVELS];
+  for (int sidx = 0; sidx < kSeedsPerThread; sidx++) {
+    uint32_t x = (uint32_t)r * 0x9E3779B9u + (uint32_t)(sidx * kSeedThreads + tid) * 0x85EBCA6Bu + 0x27D4EB2Fu;
+    float C = 1.0f, D[8], ms[DYPLAN_MAX_LEVELS];
 #pragma unroll
-      for (int i = 0; i < 8; i++) D[i] = 0.0f;
+    for (int i = 0; i < 8; i++) D[i] = 0.0f;
 #pragma unroll
-      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) ms[l] = slo_f;
-      for (int i = Np - 1; i >= 0; --i) {
-        x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;   // integer hash, one draw per node
-        const int kp = i == 0 ? K0p : h->Kp[i];
-        const int slot = h->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
-        C *= q_f[slot];
-        D[q_be[slot] & 7] += q_dem[slot];
-        const uint32_t dm0 = h->deps[i];
+    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) ms[l] = slo_f;
+    for (int i = Np - 1; i >= 0; --i) {
+      x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;   // integer hash, one draw per node
+      const int kp = i == 0 ? K0p : sh->Kp[i];
+      const int slot = sh->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
+      C *= p_f[slot];
+      const int be = p_be[slot] & 7;
+      const float dm = p_dem[slot];
 #pragma unroll
-        for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
-          if (l < L) {
-            float m = slo_f;
-            for (uint32_t dm = dm0; dm; dm &= dm - 1) m = fminf(m, su[__ffs(dm) - 1][l]);
-            const float v = m + q_nlat[slot * Lp + l];
-            su[i][l] = v;
-            ms[l] = fminf(ms[l], v);
-          }
+      for (int bb = 0; bb < 8; bb++) D[bb] += (bb == be) ? dm : 0.0f;
+      const uint32_t dm0 = sh->deps[i];
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+        if (l < L) {
+          float m = slo_f;
+          for (uint32_t dmk = dm0; dmk; dmk &= dmk - 1) m = fminf(m, su[__ffs(dmk) - 1][l]);
+          const float v = m + p_nlat[slot * Lp + l];
+          su[i][l] = v;
+          ms[l] = fminf(ms[l], v);
         }
       }
-      bool capok = C > 0.0f;   // a padding slot of node 0 has f = 0
-      if (nbc) for (int bb = 0; bb < B; bb++) capok &= D[bb] <= h->capf[bb];
-      if (capok) {
+    }
+    bool capok = C > 0.0f;   // a padding slot of node 0 has f = 0
+    if (nbc) {
 #pragma unroll
-        for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
-          if (l < L && ms[l] >= 0.0f) atomicMax((int*)&a.gthr[r * L + l], __float_as_int(C));
-      }
+      for (int bb = 0; bb < 8; bb++) capok &= (bb >= B) || D[bb] <= sh->capf[bb];
+    }
+    if (capok) {
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
+        if (l < L && ms[l] >= 0.0f) atomicMax((int*)&a.gthr[r * L + l], __float_as_int(C));
     }
   }
 }
@@ -477,6 +498,12 @@ cudaError_t launch_stage(const CallArgs& a, cudaStream_t s) {
   const unsigned grid = (unsigned)((a.in.R + wpb - 1) / wpb);
   if (grid == 0) return cudaSuccess;
   k_stage<<<grid, wpb * 32, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_seed(const CallArgs& a, cudaStream_t s) {
+  if (a.in.R == 0) return cudaSuccess;
+  k_seed<<<(unsigned)a.in.R, kSeedThreads, 0, s>>>(a);
   return cudaGetLastError();
 }
 
