@@ -24,6 +24,8 @@ struct __align__(16) FWarpShared {
   Best best[8];                    // the warp's incumbent per level (written by the cooperative slow path only)
   int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
   float scr[40];                   // slow path: the flagged lane's group state, broadcast through shared memory
+  float ctx[(L >= 6 ? 4 * L * 32 : 32)];   // (L >= 6 only) [4 l + v][lane]: node-2 context of every lane (X2, Rm3, U1r, A0r per level), written
+                                   // by the heavy step and read by each light step (kept out of the register file)
   unsigned long long bar;          // mbarrier of the TMA copy
   unsigned long long pad;
 };
@@ -99,7 +101,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
   int k2 = dig[2];
   int top = Np - 1;   // recompute nodes top..3
   bool need_heavy = true;
-  float X2[L], Rm3[L], U1r[L], A0r[L], D3[NBX];
+  constexpr bool kCtxShared = L >= 6;   // many levels: the node-2 context does not fit the register file beside the tables
+  float D3[NBX];
+  float X2r[L], Rm3r[L], U1rr[L], A0rr[L];   // node-2 context in registers (L < 6)
+  float* cx = ws->ctx + lane;                 // this lane's column of the node-2 context in shared memory (L >= 6)
   float C3 = 0.0f;
   float nthrm[L];   // -pred(thr_l): the screen's addend
   // lane l < Lr reads the bits of the best C the request's warps have published for level l, one light step ahead
@@ -135,7 +140,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       }
     }
 #pragma unroll
-    for (int l = 0; l < L; l++) { X2[l] = slo; U1r[l] = slo; A0r[l] = slo; Rm3[l] = Rm[3][l]; }
+    {
+    float X2[L], U1r[L], A0r[L];
+#pragma unroll
+    for (int l = 0; l < L; l++) { X2[l] = slo; U1r[l] = slo; A0r[l] = slo; }
     for (uint32_t dm = deps2; dm; dm &= dm - 1) {
       const int j = __ffs(dm) - 1;
 #pragma unroll
@@ -150,6 +158,15 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       const int j = __ffs(dm) - 1;
 #pragma unroll
       for (int l = 0; l < L; l++) A0r[l] = fminf(A0r[l], u[j][l]);
+    }
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      if (kCtxShared) {
+        cx[(4 * l + 0) * 32] = X2[l]; cx[(4 * l + 1) * 32] = Rm[3][l]; cx[(4 * l + 2) * 32] = U1r[l]; cx[(4 * l + 3) * 32] = A0r[l];
+      } else {
+        X2r[l] = X2[l]; Rm3r[l] = Rm[3][l]; U1rr[l] = U1r[l]; A0rr[l] = A0r[l];
+      }
+    }
     }
     C3 = Cp[3];
 #pragma unroll
@@ -173,10 +190,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     float R2[L], U1pS[L], A0q1[L];
 #pragma unroll
     for (int l = 0; l < L; l++) {
-      const float u2 = X2[l] + s_nlat[slot2 * L + l];
-      R2[l] = fminf(Rm3[l], u2);
-      const float U1 = fminf(U1r[l], u2 + big12);
-      const float a0 = fminf(A0r[l], u2 + big02);
+      const float u2 = (kCtxShared ? cx[(4 * l + 0) * 32] : X2r[l]) + s_nlat[slot2 * L + l];
+      R2[l] = fminf(kCtxShared ? cx[(4 * l + 1) * 32] : Rm3r[l], u2);
+      const float U1 = fminf(kCtxShared ? cx[(4 * l + 2) * 32] : U1rr[l], u2 + big12);
+      const float a0 = fminf(kCtxShared ? cx[(4 * l + 3) * 32] : A0rr[l], u2 + big02);
       A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
       U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
     }
