@@ -221,7 +221,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
-      float zm = 0.0f;
+      float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
 #pragma unroll
       for (int k0 = 0; k0 < K0P; k0++) {
         float P = C1 * f0[k0];
@@ -230,9 +230,13 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
         for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, nthrm[l]);
 #pragma unroll
-        for (int l = 0; l + 1 < L; l += 2) zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
-        if (L & 1) zm = fmaxf(zm, z[L - 1]);
+        for (int l = 0; l + 1 < L; l += 2) {
+          if (NB && (((l >> 1) + k0) & 1)) zm2 = fmaxf(zm2, fmaxf(z[l], z[l + 1]));
+          else zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
+        }
+        if (L & 1) { if (NB && (k0 & 1)) zm2 = fmaxf(zm2, z[L - 1]); else zm = fmaxf(zm, z[L - 1]); }
       }
+      zm = fmaxf(zm, zm2);
       unsigned flagged = __ballot_sync(0xffffffffu, zm > 0.0f);
       if (__builtin_expect(flagged != 0u, 0)) {
         // ---- cooperative slow path: exact order on the group of every flagged lane ----
