@@ -222,6 +222,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
       float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
+      float zodd = 0.0f;             // odd L: the last level of an even k0 waits for the one of k0 + 1 (one FMNMX3 for both)
 #pragma unroll
       for (int k0 = 0; k0 < K0P; k0++) {
         float P = C1 * f0[k0];
@@ -234,7 +235,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
           if (NB && (((l >> 1) + k0) & 1)) zm2 = fmaxf(zm2, fmaxf(z[l], z[l + 1]));
           else zm = fmaxf(zm, fmaxf(z[l], z[l + 1]));
         }
-        if (L & 1) { if (NB && (k0 & 1)) zm2 = fmaxf(zm2, z[L - 1]); else zm = fmaxf(zm, z[L - 1]); }
+        if (L & 1) {
+          if (k0 & 1) { if (NB && (k0 & 2)) zm2 = fmaxf(zm2, fmaxf(zodd, z[L - 1])); else zm = fmaxf(zm, fmaxf(zodd, z[L - 1])); }
+          else zodd = z[L - 1];
+        }
       }
       zm = fmaxf(zm, zm2);
       unsigned flagged = __ballot_sync(0xffffffffu, zm > 0.0f);
