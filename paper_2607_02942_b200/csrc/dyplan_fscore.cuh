@@ -206,6 +206,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
     }
 
+    float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
 #pragma unroll 2
     for (int k1 = 0; k1 < K1; k1++) {
       const int slot1 = K0P + k1;
@@ -221,7 +222,6 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
-      float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
       float zodd = 0.0f;             // odd L: the last level of an even k0 waits for the one of k0 + 1 (one FMNMX3 for both)
 #pragma unroll
       for (int k0 = 0; k0 < K0P; k0++) {
@@ -240,28 +240,39 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
           else zodd = z[L - 1];
         }
       }
-      zm = fmaxf(zm, zm2);
-      unsigned flagged = __ballot_sync(0xffffffffu, zm > 0.0f);
-      if (__builtin_expect(flagged != 0u, 0)) {
-        // ---- cooperative slow path: exact order on the group of every flagged lane ----
-        // (what the other warps have published by now is fetched meanwhile and applied on the way out: many flags
-        // are stale-threshold flags, and the next groups should not raise them again)
-        const int pub = __ldcg(gaddr);
-        while (flagged) {
-          const int src = __ffs(flagged) - 1;
-          flagged &= flagged - 1;
-          if (lane == src) {
-            slow_steps++;
-            ws->scr[kScrC1] = C1;
+    }
+    // one vote per light step: did any of this lane's K1 x K0P x L evaluations pass the screen?
+    unsigned flagged = __ballot_sync(0xffffffffu, fmaxf(zm, zm2) > 0.0f);
+    if (__builtin_expect(flagged != 0u, 0)) {
+      // ---- cooperative slow path: exact order on the K1 groups of every flagged lane ----
+      // (what the other warps have published by now is fetched meanwhile and applied on the way out: many flags
+      // are stale-threshold flags, and the next steps should not raise them again)
+      const int pub = __ldcg(gaddr);
+      while (flagged) {
+        const int src = __ffs(flagged) - 1;
+        flagged &= flagged - 1;
+        if (lane == src) {
+          slow_steps++;
+          ws->scr[kScrC1] = C2;
 #pragma unroll
-            for (int b = 0; b < NBX; b++) ws->scr[kScrS1 + b] = NB ? s1[b] : 0.0f;
+          for (int b = 0; b < NBX; b++) ws->scr[kScrS1 + b] = NB ? sD2[b] : 0.0f;
 #pragma unroll
-            for (int l = 0; l < L; l++) { ws->scr[kScrAp1 + l] = ap1[l]; ws->scr[kScrU1 + l] = U1pS[l]; ws->scr[kScrR2 + l] = R2[l]; }
+          for (int l = 0; l < L; l++) { ws->scr[kScrAp1 + l] = A0q1[l]; ws->scr[kScrU1 + l] = U1pS[l]; ws->scr[kScrR2 + l] = R2[l]; }
+        }
+        __syncwarp();
+        const float gC2 = ws->scr[kScrC1];
+        bool have_idx = false;
+        unsigned long long gidx2 = 0;
+        for (int k1 = 0; k1 < K1; k1++) {
+          const int slot1 = K0P + k1;
+          // the group's state, recomputed from the light-step state with the screen's own operations
+          float gC1 = __fmul_rn(gC2, s_f[slot1]);
+          if (NB) {
+            float smin = kBigF;
+#pragma unroll
+            for (int b = 0; b < NBX; b++) smin = fminf(smin, ws->scr[kScrS1 + b] - s_dem1b[k1 * 8 + b]);
+            gC1 = __fmul_rn(gC1, __saturatef(smin));
           }
-          __syncwarp();
-          const float gC1 = ws->scr[kScrC1];
-          bool have_idx = false;
-          unsigned long long gidx1 = 0;
           for (int e0 = 0; e0 < K0P * L; e0 += 32) {
             const int e = e0 + lane;
             bool cand = false;
@@ -271,10 +282,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
               k0 = e / L;
               l = e - k0 * L;
               P = __fmul_rn(gC1, s_f[k0]);
-              if (NB) P = __fmul_rn(P, __saturatef(ws->scr[kScrS1 + k0 / G] - s_dem[k0]));
-              const float t1 = ws->scr[kScrAp1 + l] + s_nlat[e];          // slack + 1 of node 0's path
-              const float u1p = fmaf(s_nlat[slot1 * L + l], S01, ws->scr[kScrU1 + l]) * rS01;   // slack + 1 of node 1
-              const float ms1 = fminf(fminf(t1, u1p), ws->scr[kScrR2 + l] + 1.0f);              // least slack + 1
+              if (NB) P = __fmul_rn(P, __saturatef((ws->scr[kScrS1 + k0 / G] - s_dem1b[k1 * 8 + k0 / G]) - s_dem[k0]));
+              const float u1pS = fmaf(s_nlat[slot1 * L + l], S01, ws->scr[kScrU1 + l]);
+              const float t1 = fminf(ws->scr[kScrAp1 + l], u1pS) + s_nlat[e];   // slack + 1 of node 0's path
+              const float ms1 = fminf(fminf(t1, u1pS * rS01), ws->scr[kScrR2 + l] + 1.0f);   // least slack + 1
               T = (int)((slo + 1.0f) - ms1);
               // phase 1: feasible, and not worse than the warp's incumbent on (C desc, T asc)
               const float bC = ((volatile float*)&ws->best[l].C)[0];
@@ -283,17 +294,17 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
             }
             unsigned cm = __ballot_sync(0xffffffffu, cand);
             if (cm && !have_idx) {
-              // phase 2 needs the canonical index of the flagged lane's prefix
+              // phase 2 needs the canonical index of the flagged lane's prefix (nodes >= 2)
               have_idx = true;
               if (lane == src) {
-                unsigned long long idx1 = h->base_idx + s_idxc[slot1] + s_idxc[slot2];
-                for (int i = 3; i < Np; i++) idx1 += s_idxc[h->optbase[i] + dig[i]];
-                *(unsigned long long*)&ws->scr[kScrIdx] = idx1;
+                unsigned long long idx2 = h->base_idx + s_idxc[slot2];
+                for (int i = 3; i < Np; i++) idx2 += s_idxc[h->optbase[i] + dig[i]];
+                *(unsigned long long*)&ws->scr[kScrIdx] = idx2;
               }
               __syncwarp();
-              gidx1 = *(const unsigned long long*)&ws->scr[kScrIdx];
+              gidx2 = *(const unsigned long long*)&ws->scr[kScrIdx];
             }
-            const unsigned long long idx = gidx1 + s_idxc[k0];
+            const unsigned long long idx = gidx2 + s_idxc[slot1] + s_idxc[k0];
             while (cm) {
               const int c = __ffs(cm) - 1;
               cm &= cm - 1;
@@ -316,15 +327,15 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
               }
             }
           }
-          __syncwarp();
         }
-        if (lane < Lr && pub > ((volatile int*)w_thr)[lane]) w_thr[lane] = pub;
         __syncwarp();
+      }
+      if (lane < Lr && pub > ((volatile int*)w_thr)[lane]) w_thr[lane] = pub;
+      __syncwarp();
 #pragma unroll
-        for (int l = 0; l < L; l++) {
-          const int t = ((volatile int*)w_thr)[l];
-          nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
-        }
+      for (int l = 0; l < L; l++) {
+        const int t = ((volatile int*)w_thr)[l];
+        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
       }
     }
     // ---- advance ----
