@@ -406,7 +406,8 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     // lanes take consecutive sub-ranges of the same length (a multiple of node 2's radix, so that every lane is at
     // the same k2 and the heavy steps coincide); every lane runs `per` steps, the ones past its range score nothing
     const unsigned long long K2u = (unsigned long long)h->Kp[2];
-    const unsigned long long per = (((len + 31) / 32 + K2u - 1) / K2u) * K2u;
+    const unsigned long long per0 = (len + 31) / 32;
+    const unsigned long long per = per0 < 4 * K2u ? per0 : ((per0 + K2u - 1) / K2u) * K2u;
     const unsigned long long tb = min(ob + (unsigned long long)lane * per, oe);
     const unsigned long long te = min(tb + per, oe);
     {

@@ -27,6 +27,7 @@ constexpr float kBigF = 16777216.0f; // 2^24
 // so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)
 __host__ __device__ inline unsigned long long fast_item_outer(unsigned long long pif, int K2) {
   const unsigned long long q = 32ull * (unsigned long long)(K2 < 1 ? 1 : K2);
+  if (pif < 4 * q) return ((pif + 31) / 32) * 32;   // small calls: favour more items over aligned lanes
   return ((pif + q - 1) / q) * q;
 }
 __host__ __device__ inline int level_class(int L) { return L <= 4 ? L : (L <= 6 ? 6 : 8); }
