@@ -103,7 +103,8 @@ class ClockSampler:
 def make_workload(cfg: int, rank: int, requests: int | None):
     from paper_2607_02942_b200 import workloads as wl
     # rank 0 runs the config's own seed; other ranks an independent batch of the same shape
-    return wl.make_config(cfg, R=requests, seed=cfg + 1000 * rank)
+    from paper_2607_02942_b200.multi import rank_seed
+    return wl.make_config(cfg, R=requests, seed=rank_seed(cfg, rank))
 
 
 def oracle_sample(w, n_req: int):
@@ -242,17 +243,15 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
     dres = dw.out.host()
     assert np.array_equal(dres["plan_idx"], pin_out["plan_idx"].numpy().view(np.uint64)), "host/device legs disagree"
 
-    if world > 1:
-        for t in (tot_ms, k_ms, e2e_t):
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    tot_ms, k_ms, e2e_ms = float(tot_ms), float(k_ms), float(e2e_t)
+    from paper_2607_02942_b200.multi import max_over_ranks, whole_job_rate
+    tot_ms, k_ms, e2e_ms = max_over_ranks([float(tot_ms), float(k_ms), float(e2e_t)], device=dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     sm_count = st["sm_count"]
-    value = world * evals * args.steps / (tot_ms * 1e-3) / 1e9
+    value = whole_job_rate(evals, world, args.steps, tot_ms) / 1e9
     k_eval_s = evals * args.steps / (k_ms * 1e-3)
     aops = alg_ops_per_eval(w)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
