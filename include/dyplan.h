@@ -134,6 +134,37 @@ DYPLAN_API int dyplan_replan(dyplan_ctx* ctx, const dyplan_batch* in, const uint
 DYPLAN_API int dyplan_select(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L,
                   const int32_t* live_mult_pm, int32_t* variant, dyplan_bundle* rescored, void* stream);
 
+/* Section 5.1 as the paper states it, one decision per request, no solver: the STATEFUL selector.
+ * Inputs per request: the index of its active variant (cur_variant, -1 = none installed yet), the time since its last
+ * switch, its dispatched-node mask and its active assignment; shared: one load figure per MODEL (the runtime
+ * "summarizes the load of replicas serving the same model").  The rule, in the paper's order:
+ *   - no active variant (or it is not OK in the bundle): install the lowest-index OK variant          -> switched = 3
+ *   - since_switch < min_dwell: retain ("a minimum dwell time between switches")         -> switched = 0
+ *   - load[dom(cur)] > hi_load: scan the LATER variants in level order; skip a candidate that is not OK, whose
+ *     dominant model is the same congested class, or is itself above hi_load; it must be sufficiently less loaded
+ *     (load[dom(k)] <= load[dom(cur)] - load_margin) and its estimated quality drop C(cur) - C(k) must not exceed
+ *     quality_tol; the FIRST candidate passing both checks is selected              -> switched = 1
+ *   - otherwise ("when load subsides"): the lowest-index EARLIER variant whose dominant-model load is below lo_load
+ *     and that passes the quality check                                                -> switched = 2
+ *   - no eligible transition: the current selection is retained                                       -> switched = 0
+ * Applying the selection (Fig. 7(c)): active_choice[n] takes the selected variant's option only for
+ * nodes whose bit in dispatched_mask is clear; dispatched nodes keep their binding.  The dominant model of a variant
+ * is bundle->dom_model (decided at compile time), its quality estimate bundle->corr64 (corr if NULL).
+ * hi_load, lo_load, load_margin, quality_tol, min_dwell are "configured" in the paper and never printed: parameters
+ * here.  A NaN load or since_switch retains the selection.  All pointers are DEVICE pointers. */
+typedef struct {
+  float hi_load;     /* high-load threshold of the active variant's dominant model                      */
+  float lo_load;     /* low-load threshold for returning to an earlier variant                          */
+  float load_margin; /* comparison rule: a candidate must be at least this much less loaded             */
+  float quality_tol; /* largest accepted drop of the estimated quality C                                */
+  float min_dwell;   /* minimum time since the request's last switch (same unit as since_switch)       */
+} dyplan_switch_params;
+
+DYPLAN_API int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L,
+                  const dyplan_switch_params* params, const float* model_load /*[M]*/, const float* since_switch /*[R]*/,
+                  const uint32_t* dispatched_mask /*[R]*/, int32_t* cur_variant /*[R] in/out*/,
+                  uint8_t* active_choice /*[R*16] in/out*/, uint8_t* switched /*[R] out*/, void* stream);
+
 /* Same three calls with HOST pointers everywhere (batch fields, multipliers, masks, outputs).  The library copies
  * inputs to the device, runs the same kernels and copies the results back, all on `stream`, and returns after a
  * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied. */

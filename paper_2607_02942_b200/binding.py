@@ -26,7 +26,7 @@ FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
 EXPORTS = (
-    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select",
+    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
 )
@@ -48,6 +48,11 @@ class CBatch(C.Structure):
 class CBundle(C.Structure):
     _fields_ = [("plan_idx", C.c_void_p), ("choice", C.c_void_p), ("corr", C.c_void_p), ("corr64", C.c_void_p),
                 ("lat", C.c_void_p), ("dem", C.c_void_p), ("dom_model", C.c_void_p), ("status", C.c_void_p)]
+
+
+class CSwitchParams(C.Structure):
+    _fields_ = [("hi_load", C.c_float), ("lo_load", C.c_float), ("load_margin", C.c_float),
+                ("quality_tol", C.c_float), ("min_dwell", C.c_float)]
 
 
 class CStats(C.Structure):
@@ -73,6 +78,7 @@ def lib():
         l.dyplan_compile.argtypes = [vp, pb, i32, vp, po, vp]
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
+        l.dyplan_switch.argtypes = [vp, pb, po, i32, C.POINTER(CSwitchParams), vp, vp, vp, vp, vp, vp, vp]
         l.dyplan_compile_host.argtypes = [vp, pb, i32, vp, po, vp, pu64, pu64]
         l.dyplan_replan_host.argtypes = [vp, pb, vp, vp, vp, u32, po, vp, pu64, pu64]
         l.dyplan_select_host.argtypes = [vp, pb, po, i32, vp, vp, po, vp, pu64, pu64]
@@ -256,6 +262,14 @@ class Context:
                                         _ptr(live_mult_pm), _ptr(variant),
                                         C.byref(rescored.cstruct) if rescored is not None else None,
                                         _stream_ptr(stream)))
+
+    def dyplan_switch(self, batch: Buffers, bundle: Buffers, L: int, params: dict, model_load, since_switch,
+                      dispatched_mask, cur_variant, active_choice, switched, stream=None):
+        p = CSwitchParams(params["hi_load"], params["lo_load"], params["load_margin"], params["quality_tol"],
+                          params["min_dwell"])
+        self._check(lib().dyplan_switch(self._h, C.byref(batch.cstruct), C.byref(bundle.cstruct), L, C.byref(p),
+                                        _ptr(model_load), _ptr(since_switch), _ptr(dispatched_mask), _ptr(cur_variant),
+                                        _ptr(active_choice), _ptr(switched), _stream_ptr(stream)))
 
     def dyplan_compile_host(self, batch: Buffers, L: int, mult_pm: np.ndarray, out: Buffers, stream=None):
         h2d, d2h = C.c_uint64(), C.c_uint64()

@@ -265,6 +265,33 @@ int dyplan_select(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* 
   return DYPLAN_OK;
 }
 
+int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L, const dyplan_switch_params* params,
+                  const float* model_load, const float* since_switch, const uint32_t* dispatched_mask, int32_t* cur_variant,
+                  uint8_t* active_choice, uint8_t* switched, void* stream) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = check_batch(in, false);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  ctx->last_launches = 0;
+  ctx->have_events = false;
+  ctx->last_stream = (cudaStream_t)stream;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!in->node_off || !params || !bundle || !bundle->choice || !bundle->status || !bundle->dom_model ||
+      (!bundle->corr64 && !bundle->corr) || !model_load || !since_switch || !dispatched_mask || !cur_variant ||
+      !active_choice || !switched)
+    return DYPLAN_ERR_NULL;
+  if (!(params->hi_load >= params->lo_load) || !(params->load_margin >= 0.0f) || !(params->quality_tol >= 0.0f))
+    return DYPLAN_ERR_ARG;
+  CK(cudaSetDevice(ctx->device));
+  SwitchArgs a;
+  memset(&a, 0, sizeof(a));
+  a.in = *in; a.bundle = *bundle; a.L = L; a.p = *params; a.model_load = model_load; a.since_switch = since_switch;
+  a.dispatched = dispatched_mask; a.cur_variant = cur_variant; a.active_choice = active_choice; a.switched = switched;
+  CK(launch_switch(a, (cudaStream_t)stream));
+  ctx->last_launches = 1;
+  return DYPLAN_OK;
+}
+
 int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
   if (!ctx || !out) return DYPLAN_ERR_NULL;
   memset(out, 0, sizeof(*out));

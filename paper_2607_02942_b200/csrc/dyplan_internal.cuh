@@ -130,6 +130,19 @@ struct SelectArgs {
   int32_t has_rescored;
 };
 cudaError_t launch_select(const SelectArgs& a, cudaStream_t s);
+struct SwitchArgs {
+  dyplan_batch in;
+  dyplan_bundle bundle;            // choice, status, dom_model, corr64 (or corr)
+  int32_t L;
+  dyplan_switch_params p;
+  const float* model_load;         // [M]
+  const float* since_switch;       // [R]
+  const uint32_t* dispatched;      // [R]
+  int32_t* cur_variant;            // [R] in/out
+  uint8_t* active_choice;          // [R*16] in/out
+  uint8_t* switched;               // [R] out
+};
+cudaError_t launch_switch(const SwitchArgs& a, cudaStream_t s);
 
 __host__ __device__ inline int nb_class_of(int B, bool has_caps) { return !has_caps ? 0 : (B <= 2 ? 2 : (B <= 4 ? 4 : 8)); }
 

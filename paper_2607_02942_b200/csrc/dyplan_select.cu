@@ -133,6 +133,71 @@ __global__ void __launch_bounds__(128) k_select(SelectArgs a) {
   }
 }
 
+// ---- K_switch: the paper's stateful load-driven selector, one thread per request.  The rule is
+// spelled out in include/dyplan.h (dyplan_switch); nothing here solves anything: it reads L records per request. ----
+__global__ void __launch_bounds__(128) k_switch(SwitchArgs a) {
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const dyplan_batch& b = a.in;
+  if (r >= b.R) return;
+  const int L = a.L, M = b.M;
+  const dyplan_bundle& v = a.bundle;
+  const long long rec0 = r * L;
+  const int cur = a.cur_variant[r];
+  int pick = cur;
+  int how = 0;
+  auto okv = [&](int k) { return v.status[rec0 + k] == DYPLAN_ST_OK && v.dom_model[rec0 + k] < M; };
+  auto qual = [&](int k) { return v.corr64 ? v.corr64[rec0 + k] : (double)v.corr[rec0 + k]; };
+  auto load = [&](int k) { return a.model_load[v.dom_model[rec0 + k]]; };
+  if (cur < 0 || cur >= L || !okv(cur)) {
+    pick = -1;
+    for (int k = 0; k < L; k++) if (okv(k)) { pick = k; how = 3; break; }
+  } else {
+    const float dwell = a.since_switch[r];
+    const float lc = load(cur);
+    const double qc = qual(cur);
+    if (dwell >= a.p.min_dwell && lc == lc) {   // NaN dwell or load: retain
+      if (lc > a.p.hi_load) {
+        const int dc = v.dom_model[rec0 + cur];
+        for (int k = cur + 1; k < L; k++) {
+          if (!okv(k)) continue;
+          if (v.dom_model[rec0 + k] == dc) continue;          // the same congested class
+          const float lk = load(k);
+          if (!(lk <= a.p.hi_load)) continue;                   // itself overloaded (or NaN)
+          if (!((double)lk <= (double)lc - (double)a.p.load_margin)) continue;   // not sufficiently less loaded
+          if (!(qc - qual(k) <= (double)a.p.quality_tol)) continue;
+          pick = k; how = 1;
+          break;
+        }
+      } else {
+        for (int k = 0; k < cur; k++) {
+          if (!okv(k)) continue;
+          if (!(load(k) < a.p.lo_load)) continue;
+          if (!(qc - qual(k) <= (double)a.p.quality_tol)) continue;
+          pick = k; how = 2;
+          break;
+        }
+      }
+    }
+  }
+  if (pick != cur && pick >= 0) {
+    // node-boundary safe point: only undispatched nodes take the selected variant's bindings
+    const uint32_t dm = a.dispatched[r];
+    const int N = b.node_off[r + 1] - b.node_off[r];
+    const uint8_t* ch = v.choice + (rec0 + pick) * 16;
+    for (int n = 0; n < 16; n++)
+      if (n < N && !((dm >> n) & 1)) a.active_choice[r * 16 + n] = ch[n];
+  }
+  a.cur_variant[r] = pick;
+  a.switched[r] = (uint8_t)(pick != cur ? how : 0);
+}
+
+cudaError_t launch_switch(const SwitchArgs& a, cudaStream_t s) {
+  const unsigned grid = (unsigned)((a.in.R + 127) / 128);
+  if (grid == 0) return cudaSuccess;
+  k_switch<<<grid, 128, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_select(const SelectArgs& a, cudaStream_t s) {
   const unsigned grid = (unsigned)((a.in.R + 127) / 128);
   if (grid == 0) return cudaSuccess;

@@ -364,6 +364,55 @@ def test_select_parity(dy, orc, seed):
         assert np.array_equal(vh, v)
 
 
+# ---- the paper's stateful selector: dyplan_switch against oracle/switch_oracle.py ---------------
+@pytest.mark.parametrize("seed", [111, 112, 113])
+def test_switch_parity(dy, orc, seed):
+    import torch
+    from oracle import switch_oracle as so
+    binding, ctx = dy
+    L, B, M, R = 5, 3, 4, 300
+    w = wl.random_workload(seed, R=R, nmin=1, nmax=8, kmin=1, kmax=4, B=B, M=M, L=L, caps=True, slo_q=0.35)
+    w.batch.vuln[w.batch.node_off[7]] = np.nan                 # one request without any plan
+    ref = orc.run(w)                                           # the bundle comes from the oracle, not from the GPU
+    bundle_host = dict(plan_idx=ref["plan_idx"], choice=ref["choice"], corr=ref["corr"].astype(np.float32),
+                       corr64=ref["corr"], lat=np.minimum(ref["lat"], 2**31 - 1).astype(np.int32), dem=ref["dem"],
+                       dom_model=ref["dom_model"], status=ref["status"])
+    dbundle = binding.bundle_from_host(bundle_host, R, L, B, "cuda:0")
+    dbatch = binding.make_batch(w.batch, "cuda:0")
+    rng = np.random.default_rng(seed)
+    n_nodes = np.array([w.batch.n_nodes(r) for r in range(R)])
+    f32 = lambda x: float(np.float32(x))
+    seen = set()
+    for trial in range(6):
+        params = dict(hi_load=f32(rng.uniform(0.5, 0.9)), lo_load=f32(rng.uniform(0.1, 0.5)),
+                      load_margin=f32(rng.uniform(0.0, 0.3)), quality_tol=f32(rng.uniform(0.0, 0.2)),
+                      min_dwell=f32(rng.uniform(0.0, 5.0)))
+        load = rng.uniform(0.0, 1.2, size=M).astype(np.float32)
+        if trial == 4:
+            load[1] = np.nan
+        cur = rng.integers(-1, L, size=R).astype(np.int32)
+        since = rng.uniform(0.0, 10.0, size=R).astype(np.float32)
+        disp = np.array([rng.integers(0, 1 << n) if n else 0 for n in n_nodes], dtype=np.uint32)
+        active = rng.integers(0, 4, size=R * 16).astype(np.uint8)
+        exp = so.switch(R, L, n_nodes, ref["status"], ref["dom_model"], ref["corr"], ref["choice"], load, cur, since,
+                        disp, active, params)
+        t = lambda a: torch.from_numpy(a.view(np.int32) if a.dtype == np.uint32 else a).cuda()
+        d_cur, d_act = t(cur.copy()), t(active.copy())
+        d_sw = torch.full((R,), 77, dtype=torch.uint8, device="cuda")
+        ctx.dyplan_switch(dbatch, dbundle, L, params, t(load), t(since), t(disp), d_cur, d_act, d_sw)
+        torch.cuda.synchronize()
+        assert np.array_equal(d_cur.cpu().numpy(), exp["variant"]), trial
+        assert np.array_equal(d_sw.cpu().numpy(), exp["switched"]), trial
+        assert np.array_equal(d_act.cpu().numpy(), exp["active"]), trial
+        seen |= set(exp["switched"].tolist())
+    assert seen == {0, 1, 2, 3}                                # every branch of the rule was reached
+    # argument checks
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_switch(dbatch, dbundle, L, dict(params, hi_load=0.1, lo_load=0.5), t(load), t(since), t(disp), d_cur,
+                          d_act, d_sw)
+    assert e.value.code == binding.ERR_ARG
+
+
 def test_api_argument_errors(dy):
     binding, ctx = dy
     w = wl.random_workload(81, R=2, nmin=2, nmax=3, kmin=2, kmax=3, B=2, M=2, L=2, caps=False)
