@@ -139,7 +139,6 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
         for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0.0f);
       }
     }
-#pragma unroll
     {
     float X2[L], U1r[L], A0r[L];
 #pragma unroll

@@ -28,7 +28,8 @@ def test_header_declares_the_three_calls():
     names = declared()
     for n in ("dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_create", "dyplan_destroy"):
         assert n in names
-    assert len(names) == 12
+    assert "dyplan_switch" in names
+    assert len(names) == 13
 
 
 def test_library_exports_every_declared_symbol(binding):
