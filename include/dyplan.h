@@ -165,6 +165,34 @@ DYPLAN_API int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dypl
                   const uint32_t* dispatched_mask /*[R]*/, int32_t* cur_variant /*[R] in/out*/,
                   uint8_t* active_choice /*[R*16] in/out*/, uint8_t* switched /*[R] out*/, void* stream);
 
+/* The paper's own objective ("linear mode", Eq.(4)/(5)) over the same plan space, by exhaustive
+ * enumeration: for every level L_k maximise
+ *     J_L(pi) = sum_n [ rho(n) q - lambda_f v_n (1 - q) - lambda_c c ](n, k_n)  -  lambda_l T(pi)  -  lambda_ld L D_tau(pi)
+ * with rho(n) = 1 + beta e (|R(n)| - 1) / (|V| - 1) (rho = 1 for one node; R(n) = n and everything reachable from it,
+ * PAPER.md:178), T the longest path of the NOMINAL durations tau (Eq.(3); no pressure multipliers here: the paper's
+ * levels weight a demand penalty) and D_tau = sum_n tau(n, k_n).  Ties: T ascending, then canonical
+ * index ascending.  Reads in->lat_us (tau), in->acc (q), in->vuln (v), in->demand / backend / model (annotations);
+ * in->slo_us and in->cap are ignored (the paper's latency charge is soft).  cost: [KK] DEVICE pointer, c >= 0.
+ * params and levels are HOST pointers (levels[L], ascending from 0 in the paper; any finite values >= 0 accepted).
+ * out: one record per (request, level); corr = J as the scorer computed it (fp32), corr64 = J re-evaluated in fp64,
+ * lat = T, dem / dom_model as in dyplan_compile.  extra (optional, DEVICE arrays): dtau [R*L] = D_tau of the chosen
+ * plan, quality [R*L] = prod_n (1 - v_n (1 - q)) of the chosen plan (the variant's quality estimate dyplan_switch uses).
+ * A request whose duration sum exceeds 2^22 (the scorer keeps T and D_tau as exact fp32 integers) or whose plan space
+ * exceeds 2^40 gets status TOO_LARGE; malformed requests get INVALID; the rest of the batch still compiles. */
+typedef struct {
+  float lambda_f, lambda_c, lambda_l, lambda_ld; /* weights of impact-weighted error, call cost, latency, demand */
+  float beta, effort;                            /* reach-weight magnitude and effort e in [0,1]                 */
+} dyplan_linear_params;
+
+typedef struct {
+  int32_t* dtau;   /* [R*L] or NULL */
+  double* quality; /* [R*L] or NULL */
+} dyplan_linear_extra;
+
+DYPLAN_API int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* cost,
+                          const dyplan_linear_params* params, int32_t L, const float* levels, dyplan_bundle* out,
+                          const dyplan_linear_extra* extra, void* stream);
+
 /* Same three calls with HOST pointers everywhere (batch fields, multipliers, masks, outputs).  The library copies
  * inputs to the device, runs the same kernels and copies the results back, all on `stream`, and returns after a
  * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied. */

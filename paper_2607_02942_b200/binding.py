@@ -26,7 +26,7 @@ FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
 EXPORTS = (
-    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch",
+    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
 )
@@ -55,6 +55,14 @@ class CSwitchParams(C.Structure):
                 ("quality_tol", C.c_float), ("min_dwell", C.c_float)]
 
 
+class CLinearParams(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("lambda_f", "lambda_c", "lambda_l", "lambda_ld", "beta", "effort")]
+
+
+class CLinearExtra(C.Structure):
+    _fields_ = [("dtau", C.c_void_p), ("quality", C.c_void_p)]
+
+
 class CStats(C.Structure):
     _fields_ = [("plans", C.c_uint64), ("evals", C.c_uint64), ("work_items", C.c_uint64), ("slow_steps", C.c_uint64),
                 ("fast_requests", C.c_uint64), ("launches", C.c_int32), ("sm_count", C.c_int32), ("score_ms", C.c_float)]
@@ -78,6 +86,7 @@ def lib():
         l.dyplan_compile.argtypes = [vp, pb, i32, vp, po, vp]
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
+        l.dyplan_compile_linear.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp]
         l.dyplan_switch.argtypes = [vp, pb, po, i32, C.POINTER(CSwitchParams), vp, vp, vp, vp, vp, vp, vp]
         l.dyplan_compile_host.argtypes = [vp, pb, i32, vp, po, vp, pu64, pu64]
         l.dyplan_replan_host.argtypes = [vp, pb, vp, vp, vp, u32, po, vp, pu64, pu64]
@@ -262,6 +271,15 @@ class Context:
                                         _ptr(live_mult_pm), _ptr(variant),
                                         C.byref(rescored.cstruct) if rescored is not None else None,
                                         _stream_ptr(stream)))
+
+    def dyplan_compile_linear(self, batch: Buffers, cost, params: dict, levels, out: Buffers, dtau=None, quality=None,
+                              stream=None):
+        p = CLinearParams(*[float(params[n]) for n, _ in CLinearParams._fields_])
+        lv = np.ascontiguousarray(levels, np.float32)
+        ex = CLinearExtra(_ptr(dtau), _ptr(quality))
+        self._check(lib().dyplan_compile_linear(self._h, C.byref(batch.cstruct), _ptr(cost), C.byref(p), int(lv.size),
+                                                lv.ctypes.data_as(C.c_void_p), C.byref(out.cstruct), C.byref(ex),
+                                                _stream_ptr(stream)))
 
     def dyplan_switch(self, batch: Buffers, bundle: Buffers, L: int, params: dict, model_load, since_switch,
                       dispatched_mask, cur_variant, active_choice, switched, stream=None):

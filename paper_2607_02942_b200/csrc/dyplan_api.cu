@@ -63,6 +63,8 @@ struct dyplan_ctx {
   char errbuf[256] = {0};
   // scratch
   DevBuf blob, item_off, done, gthr, partial, state;   // item_off holds both classes' offset arrays
+  DevBuf lin_blob, lin_gj, lin_gkey, lin_misc;          // linear mode
+  bool last_linear = false;
   // staging for the *_host calls: one device arena, one pinned-or-not host side is the caller's
   DevBuf arena;
   // occupancy cache [L-1][nb index]
@@ -138,7 +140,8 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
 int dyplan_destroy(dyplan_ctx* ctx) {
   if (!ctx) return DYPLAN_ERR_NULL;
   cudaSetDevice(ctx->device);
-  DevBuf* bufs[] = {&ctx->blob, &ctx->item_off, &ctx->done, &ctx->gthr, &ctx->partial, &ctx->state, &ctx->arena};
+  DevBuf* bufs[] = {&ctx->blob, &ctx->item_off, &ctx->done, &ctx->gthr, &ctx->partial, &ctx->state, &ctx->arena,
+                    &ctx->lin_blob, &ctx->lin_gj, &ctx->lin_gkey, &ctx->lin_misc};
   for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
@@ -179,6 +182,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   ctx->have_events = false;
   ctx->last_stream = stream;
   ctx->last_L = L;
+  ctx->last_linear = false;
   if (in->R == 0) return DYPLAN_OK;
   if (!mult) return DYPLAN_ERR_NULL;
   if (is_replan && (!dispatched || (in->NN > 0 && !fixed_choice))) return DYPLAN_ERR_NULL;
@@ -292,6 +296,50 @@ int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* 
   return DYPLAN_OK;
 }
 
+int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* cost, const dyplan_linear_params* params, int32_t L,
+                          const float* levels, dyplan_bundle* out, const dyplan_linear_extra* extra, void* stream) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = check_batch(in, true);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  cudaStream_t s = (cudaStream_t)stream;
+  ctx->last_launches = 0;
+  ctx->have_events = false;
+  ctx->last_stream = s;
+  ctx->last_L = L;
+  ctx->last_linear = true;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!params || !levels || (in->KK > 0 && !cost)) return DYPLAN_ERR_NULL;
+  if ((rc = check_bundle(out))) return rc;
+  const float pv[6] = {params->lambda_f, params->lambda_c, params->lambda_l, params->lambda_ld, params->beta, params->effort};
+  for (float v : pv) if (!(v >= 0.0f) || v > 1e30f) return DYPLAN_ERR_ARG;
+  if (params->effort > 1.0f) return DYPLAN_ERR_ARG;
+  for (int l = 0; l < L; l++) if (!(levels[l] >= 0.0f) || levels[l] > 1e30f) return DYPLAN_ERR_ARG;
+  CK(cudaSetDevice(ctx->device));
+  const size_t R = (size_t)in->R;
+  if ((rc = ensure(ctx, ctx->lin_blob, R * kLinBlobWords * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->lin_gj, R * L * 4))) return rc;
+  if ((rc = ensure(ctx, ctx->lin_gkey, R * L * 8))) return rc;
+  if ((rc = ensure(ctx, ctx->lin_misc, 64))) return rc;
+  LinArgs a;
+  memset(&a, 0, sizeof(a));
+  a.in = *in; a.out = *out; if (extra) a.extra = *extra; a.cost = cost; a.p = *params; a.L = L;
+  for (int l = 0; l < L; l++) a.levels[l] = levels[l];
+  a.blob = (uint32_t*)ctx->lin_blob.p; a.gJ = (int32_t*)ctx->lin_gj.p; a.gKey = (unsigned long long*)ctx->lin_gkey.p;
+  a.counter = (uint32_t*)ctx->lin_misc.p; a.plans = (unsigned long long*)((char*)ctx->lin_misc.p + 16);
+  const int grid = ctx->sm_count * 8;                         // persistent-ish: work pulled from a device counter
+  const uint32_t want = (uint32_t)grid * 4u * 16u;            // ~16 work items per resident warp
+  uint32_t chunks = (uint32_t)((want + R - 1) / R);
+  a.chunks = chunks < 1 ? 1 : (chunks > 65536u ? 65536u : chunks);
+  CK(cudaMemsetAsync(ctx->lin_misc.p, 0, 64, s));
+  CK(cudaEventRecord(ctx->ev0, s));
+  CK(launch_linear(a, grid, s));
+  CK(cudaEventRecord(ctx->ev1, s));
+  ctx->have_events = true;
+  ctx->last_launches = 4;
+  return DYPLAN_OK;
+}
+
 int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
   if (!ctx || !out) return DYPLAN_ERR_NULL;
   memset(out, 0, sizeof(*out));
@@ -299,7 +347,15 @@ int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
   out->launches = ctx->last_launches;
   CK(cudaSetDevice(ctx->device));
   CK(cudaStreamSynchronize(ctx->last_stream));
-  if (ctx->have_events && ctx->state.p) {
+  if (ctx->have_events && ctx->last_linear && ctx->lin_misc.p) {
+    unsigned long long plans = 0;
+    CK(cudaMemcpy(&plans, (char*)ctx->lin_misc.p + 16, 8, cudaMemcpyDeviceToHost));
+    out->plans = plans;
+    out->evals = plans * (uint64_t)ctx->last_L;
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    out->score_ms = ms;
+  } else if (ctx->have_events && ctx->state.p) {
     CallState st;
     CK(cudaMemcpy(&st, ctx->state.p, sizeof(st), cudaMemcpyDeviceToHost));
     out->plans = st.total_plans;

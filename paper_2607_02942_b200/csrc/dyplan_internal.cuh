@@ -144,6 +144,39 @@ struct SwitchArgs {
 };
 cudaError_t launch_switch(const SwitchArgs& a, cudaStream_t s);
 
+// ---- linear mode (dyplan_linear.cu) ----
+constexpr int kLinHdrWords = 88;                        // LinHdr size in words
+constexpr int kLinBlobWords = kLinHdrWords + 2 * (16 * 16 + 2);   // header + w[slot] + d[slot]
+struct LinHdr {
+  int32_t status;                 // DYPLAN_ST_OK / _INVALID / _TOO_LARGE
+  int32_t n_orig, n_int;          // real nodes, nodes incl. dummies (>= 2)
+  int32_t pad0;
+  unsigned long long outer_total; // prod_{i>=2} K_i
+  unsigned long long pad1;
+  int32_t K[16];                  // options per internal node (1 for dummies)
+  uint32_t succ[16];              // successor mask per node (all bits > i)
+  int32_t optbase[16];            // first table slot of node i
+  unsigned long long stride[16];  // canonical stride (0 for dummies)
+};
+static_assert(sizeof(LinHdr) == kLinHdrWords * 4, "LinHdr layout");
+struct LinArgs {
+  dyplan_batch in;
+  dyplan_bundle out;
+  dyplan_linear_extra extra;
+  const float* cost;
+  dyplan_linear_params p;
+  int32_t L;
+  float levels[DYPLAN_MAX_LEVELS];
+  // scratch
+  uint32_t* blob;                 // [R][kLinBlobWords]
+  int32_t* gJ;                    // [R*L] best J (order-preserving int encoding)
+  unsigned long long* gKey;       // [R*L] (T << 40 | idx) of the winner among the plans with J == best
+  uint32_t* counter;              // [2] dynamic work counters of the two passes
+  uint32_t chunks;                // work items per request
+  unsigned long long* plans;      // [1] total plans enumerated (stats)
+};
+cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s);
+
 __host__ __device__ inline int nb_class_of(int B, bool has_caps) { return !has_caps ? 0 : (B <= 2 ? 2 : (B <= 4 ? 4 : 8)); }
 
 }  // namespace dyplan

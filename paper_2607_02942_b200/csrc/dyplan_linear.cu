@@ -1,0 +1,291 @@
+// dyplan_linear.cu -- the paper's own objective over the same plan space (include/dyplan.h
+// dyplan_compile_linear): J_L = sum_n w(n,k_n) - lambda_l T - lambda_ld L D_tau, Eq.(4)/(5) PAPER.md:197-205.
+//
+//   k_lstage  one thread per request: validation, reach weights rho(n), w = rho q - lambda_f v (1-q)
+//             - lambda_c c per option, durations as exact fp32 integers
+//   k_lscore  two passes over every plan, one warp per work item (a range of outer indices of one request):
+//             pass 1 reduces max J per (request, level) (atomicMax on an order-preserving int encoding);
+//             pass 2 re-enumerates and reduces min (T, canonical index) over the plans whose J equals that maximum
+//             bit for bit (same instruction sequence), one 64-bit atomicMin of T << 40 | idx.  No thresholds, no slow path.
+//   k_lemit   one thread per (request, level): decode the winner, annotate, re-evaluate J in fp64
+// J32 is a pure function of the plan: W is summed from the last node down, then one FFMA per term.
+#include "dyplan_common.cuh"
+
+namespace dyplan {
+
+__device__ __forceinline__ int enc_f32(float f) { int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
+__device__ __forceinline__ float dec_f32(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
+
+__global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const dyplan_batch& b = a.in;
+  if (r >= b.R) return;
+  const int L = a.L;
+  uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
+  LinHdr* h = (LinHdr*)blob;
+  float* t_w = (float*)(blob + kLinHdrWords);
+  float* t_d = t_w + (16 * 16 + 2);
+  for (int l = 0; l < L; l++) { a.gJ[r * L + l] = INT32_MIN; a.gKey[r * L + l] = ~0ull; }
+
+  int st = DYPLAN_ST_OK;
+  const int n0 = b.node_off[r], n1 = b.node_off[r + 1], N = n1 - n0;
+  if (N < 0 || N > DYPLAN_MAX_NODES || n0 < 0 || n1 > b.NN) st = DYPLAN_ST_INVALID;
+  unsigned long long P = 1, dsum = 0;
+  if (st == DYPLAN_ST_OK) {
+    for (int n = 0; n < N && st == DYPLAN_ST_OK; n++) {
+      const int ob = b.opt_off[n0 + n], K = b.opt_off[n0 + n + 1] - ob;
+      if (K < 1 || K > DYPLAN_MAX_OPTS || ob < 0 || ob + K > b.KK) { st = DYPLAN_ST_INVALID; break; }
+      const uint32_t pm = b.pred_mask[n0 + n];
+      const float v = b.vuln[n0 + n];
+      if ((pm >> n) != 0 || !(v >= 0.0f && v <= 1.0f)) { st = DYPLAN_ST_INVALID; break; }
+      int mx = 0;
+      for (int k = 0; k < K; k++) {
+        const int o = ob + k;
+        const float q = b.acc[o], c = a.cost[o];
+        if (b.lat_us[o] < 0 || !(q >= 0.0f && q <= 1.0f) || !(c >= 0.0f) || isinf(c) || b.demand[o] < 0 ||
+            b.backend[o] >= b.B || b.model[o] >= b.M) { st = DYPLAN_ST_INVALID; break; }
+        mx = b.lat_us[o] > mx ? b.lat_us[o] : mx;
+      }
+      dsum += (unsigned long long)mx;
+      if (P > ((1ull << DYPLAN_MAX_PLANS_LOG2) / (unsigned long long)K)) { if (st == DYPLAN_ST_OK) st = DYPLAN_ST_TOO_LARGE; }
+      else P *= (unsigned long long)K;
+    }
+    if (st == DYPLAN_ST_OK && dsum > (1ull << 22)) st = DYPLAN_ST_TOO_LARGE;
+  }
+  h->status = st; h->n_orig = N; h->n_int = N < 2 ? 2 : N; h->pad0 = 0;
+  if (st != DYPLAN_ST_OK) {
+    h->outer_total = 0;
+    for (int l = 0; l < L; l++) {
+      const long long rec = r * L + l;
+      const dyplan_bundle& o = a.out;
+      o.plan_idx[rec] = kNoIdx;
+      for (int i = 0; i < 16; i++) o.choice[rec * 16 + i] = 0xFF;
+      o.corr[rec] = -1.0f;
+      if (o.corr64) o.corr64[rec] = -1.0;
+      o.lat[rec] = INT32_MAX;
+      for (int bb = 0; bb < b.B; bb++) o.dem[rec * b.B + bb] = 0;
+      o.dom_model[rec] = 0xFF;
+      o.status[rec] = (uint8_t)st;
+      if (a.extra.dtau) a.extra.dtau[rec] = 0;
+      if (a.extra.quality) a.extra.quality[rec] = -1.0;
+    }
+    return;
+  }
+  // reach sets: R(n) = {n} u R(successors), successors have larger indices
+  uint32_t reach[16], succ[16];
+  for (int n = 0; n < 16; n++) { reach[n] = 0; succ[n] = 0; }
+  for (int s = 0; s < N; s++) {
+    const uint32_t pm = b.pred_mask[n0 + s];
+    for (int n = 0; n < s; n++) if ((pm >> n) & 1) succ[n] |= 1u << s;
+  }
+  for (int n = N - 1; n >= 0; n--) {
+    uint32_t m = 1u << n;
+    for (int s = n + 1; s < N; s++) if ((succ[n] >> s) & 1) m |= reach[s];
+    reach[n] = m;
+  }
+  unsigned long long stride = 1, outer = 1;
+  int slot = 0;
+  const int Np = N < 2 ? 2 : N;
+  for (int n = 0; n < 16; n++) {
+    if (n < N) {
+      const int ob = b.opt_off[n0 + n], K = b.opt_off[n0 + n + 1] - ob;
+      const double rho = N > 1 ? 1.0 + (double)a.p.beta * (double)a.p.effort * (double)(__popc(reach[n]) - 1) / (double)(N - 1) : 1.0;
+      const double v = (double)b.vuln[n0 + n];
+      h->K[n] = K; h->succ[n] = succ[n]; h->optbase[n] = slot; h->stride[n] = stride;
+      for (int k = 0; k < K; k++) {
+        const double q = (double)b.acc[ob + k];
+        t_w[slot + k] = (float)(rho * q - (double)a.p.lambda_f * v * (1.0 - q) - (double)a.p.lambda_c * (double)a.cost[ob + k]);
+        t_d[slot + k] = (float)b.lat_us[ob + k];
+      }
+      slot += K;
+      stride *= (unsigned long long)K;
+      if (n >= 2) outer *= (unsigned long long)K;
+    } else {
+      h->K[n] = 1; h->succ[n] = 0; h->optbase[n] = slot; h->stride[n] = 0;
+      if (n < Np) { t_w[slot] = 0.0f; t_d[slot] = 0.0f; slot += 1; }   // dummy node: one neutral option
+    }
+  }
+  h->outer_total = outer;
+  atomicAdd(a.plans, P);
+}
+
+// One warp per work item (request r, chunk c): outer indices [c*per, (c+1)*per) of the request, split over the lanes.
+template <int PASS>
+__global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
+  const int lane = threadIdx.x & 31;
+  const int L = a.L;
+  const uint32_t total = (uint32_t)a.in.R * a.chunks;
+  float cl[DYPLAN_MAX_LEVELS];
+#pragma unroll
+  for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) cl[l] = l < L ? -(a.p.lambda_ld * a.levels[l]) : 0.0f;
+  const float lam_l = a.p.lambda_l;
+  for (;;) {
+    uint32_t item = 0;
+    if (lane == 0) item = atomicAdd(&a.counter[PASS], 1u);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= total) break;
+    const long long r = item / a.chunks;
+    const uint32_t c = item % a.chunks;
+    const uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
+    const LinHdr* h = (const LinHdr*)blob;
+    if (h->status != DYPLAN_ST_OK) continue;
+    const float* t_w = (const float*)(blob + kLinHdrWords);
+    const float* t_d = t_w + (16 * 16 + 2);
+    const unsigned long long outer = h->outer_total;
+    const unsigned long long per = (outer + a.chunks - 1) / a.chunks;
+    const unsigned long long cb = min((unsigned long long)c * per, outer), ce = min(cb + per, outer);
+    const unsigned long long lper = (ce - cb + 31) / 32;
+    const unsigned long long ob = min(cb + lane * lper, ce), oe = min(ob + lper, ce);
+    const int Np = h->n_int, K0 = h->K[0], K1 = h->K[1];
+    const uint32_t succ0 = h->succ[0], succ1 = h->succ[1];
+    const bool conn01 = (succ0 >> 1) & 1;
+    const unsigned long long st0 = h->stride[0], st1 = h->stride[1];
+    const int ob1 = h->optbase[1];
+
+    float best[DYPLAN_MAX_LEVELS], tgt[DYPLAN_MAX_LEVELS];
+    unsigned long long kmin[DYPLAN_MAX_LEVELS];
+#pragma unroll
+    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+      best[l] = -INFINITY; kmin[l] = ~0ull;
+      tgt[l] = (PASS == 1 && l < L) ? dec_f32(__ldcg(&a.gJ[r * L + l])) : 0.0f;
+    }
+    float u[16];
+    for (unsigned long long o = ob; o < oe; o++) {
+      // digits of the nodes >= 2, their slack DP from the last node down (u[i] = min(0, min_succ u[j]) - d: T = -min u)
+      unsigned long long t = o, idxo = 0;
+      int dig[16];
+      for (int i = 2; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
+      float Wp = 0.0f, Dp = 0.0f, Rm = 0.0f;
+      for (int i = Np - 1; i >= 2; --i) {
+        const int slot = h->optbase[i] + dig[i];
+        float m = 0.0f;
+        for (uint32_t dm = h->succ[i]; dm; dm &= dm - 1) m = fminf(m, u[__ffs(dm) - 1]);
+        const float d = t_d[slot];
+        u[i] = m - d;
+        Rm = fminf(Rm, u[i]);
+        Wp += t_w[slot];
+        Dp += d;
+      }
+      float u1in = 0.0f, a0in = 0.0f;
+      for (uint32_t dm = succ1; dm; dm &= dm - 1) u1in = fminf(u1in, u[__ffs(dm) - 1]);
+      for (uint32_t dm = succ0 & ~3u; dm; dm &= dm - 1) a0in = fminf(a0in, u[__ffs(dm) - 1]);
+      for (int k1 = 0; k1 < K1; k1++) {
+        const float d1 = t_d[ob1 + k1];
+        const float u1 = u1in - d1;
+        const float R1 = fminf(Rm, u1);
+        const float W1 = Wp + t_w[ob1 + k1];
+        const float D1 = Dp + d1;
+        const float ap = conn01 ? fminf(a0in, u1) : a0in;
+        const unsigned long long idx1 = idxo + (unsigned long long)k1 * st1;
+        for (int k0 = 0; k0 < K0; k0++) {
+          const float d0 = t_d[k0];
+          const float m = fminf(R1, ap - d0);          // least slack = -T
+          const float W0 = W1 + t_w[k0];
+          const float D0 = D1 + d0;
+          const float Jb = fmaf(lam_l, m, W0);         // W - lambda_l T
+#pragma unroll
+          for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+            if (l < L) {
+              const float J = fmaf(cl[l], D0, Jb);     // ... - lambda_ld L D_tau
+              if (PASS == 0) best[l] = fmaxf(best[l], J);
+              else if (J == tgt[l]) {
+                const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
+                kmin[l] = key < kmin[l] ? key : kmin[l];
+              }
+            }
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+      if (l < L) {
+        if (PASS == 0) {
+          float v = best[l];
+#pragma unroll
+          for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
+          if (lane == 0 && v > -INFINITY) atomicMax(&a.gJ[r * L + l], enc_f32(v));
+        } else {
+          unsigned long long v = kmin[l];
+#pragma unroll
+          for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, v, off); v = o2 < v ? o2 : v; }
+          if (lane == 0 && v != ~0ull) atomicMin(&a.gKey[r * L + l], v);
+        }
+      }
+    }
+  }
+}
+
+// One thread per (request, level): decode the winner, annotate, re-evaluate J in fp64 (definition order of the oracle:
+// W summed in node order, then - lambda_l T - lambda_ld L D_tau; no contraction).
+__global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
+  const long long rec = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const dyplan_batch& b = a.in;
+  const int L = a.L, B = b.B, M = b.M;
+  if (rec >= (long long)b.R * L) return;
+  const long long r = rec / L;
+  const int l = (int)(rec % L);
+  const LinHdr* h = (const LinHdr*)(a.blob + (size_t)r * kLinBlobWords);
+  if (h->status != DYPLAN_ST_OK) return;   // sentinels were written by k_lstage
+  const dyplan_bundle& o = a.out;
+  const unsigned long long key = a.gKey[rec];
+  unsigned long long idx = key & ((1ull << 40) - 1);
+  const int n0 = b.node_off[r], N = h->n_orig;
+  uint32_t reach[16], succ[16];
+  for (int n = 0; n < 16; n++) succ[n] = 0;
+  for (int s = 0; s < N; s++) { const uint32_t pm = b.pred_mask[n0 + s]; for (int n = 0; n < s; n++) if ((pm >> n) & 1) succ[n] |= 1u << s; }
+  for (int n = N - 1; n >= 0; n--) { uint32_t m = 1u << n; for (int s = n + 1; s < N; s++) if ((succ[n] >> s) & 1) m |= reach[s]; reach[n] = m; }
+  int D[DYPLAN_MAX_BACKENDS], Dm[DYPLAN_MAX_MODELS];
+  for (int i = 0; i < DYPLAN_MAX_BACKENDS; i++) D[i] = 0;
+  for (int i = 0; i < DYPLAN_MAX_MODELS; i++) Dm[i] = 0;
+  long long fin[16], T = 0, Dt = 0;
+  double W = 0.0, qual = 1.0;
+  o.plan_idx[rec] = idx;
+  for (int n = 0; n < 16; n++) {
+    if (n >= N) { o.choice[rec * 16 + n] = 0xFF; continue; }
+    const int ob = b.opt_off[n0 + n];
+    const unsigned long long K = (unsigned long long)(b.opt_off[n0 + n + 1] - ob);
+    const int k = (int)(idx % K);
+    idx /= K;
+    o.choice[rec * 16 + n] = (uint8_t)k;
+    const int op = ob + k;
+    const double rho = N > 1 ? __dadd_rn(1.0, __ddiv_rn(__dmul_rn(__dmul_rn((double)a.p.beta, (double)a.p.effort), (double)(__popc(reach[n]) - 1)), (double)(N - 1))) : 1.0;
+    const double q = (double)b.acc[op], v = (double)b.vuln[n0 + n];
+    const double term = __dsub_rn(__dsub_rn(__dmul_rn(rho, q), __dmul_rn(__dmul_rn((double)a.p.lambda_f, v), __dsub_rn(1.0, q))),
+                                  __dmul_rn((double)a.p.lambda_c, (double)a.cost[op]));
+    W = __dadd_rn(W, term);
+    qual = __dmul_rn(qual, __dsub_rn(1.0, __dmul_rn(v, __dsub_rn(1.0, q))));
+    long long start = 0;
+    const uint32_t pm = b.pred_mask[n0 + n];
+    for (int uu = 0; uu < n; uu++) if ((pm >> uu) & 1) start = fin[uu] > start ? fin[uu] : start;
+    fin[n] = start + b.lat_us[op];
+    T = fin[n] > T ? fin[n] : T;
+    Dt += b.lat_us[op];
+    D[b.backend[op]] += b.demand[op];
+    Dm[b.model[op]] += b.demand[op];
+  }
+  int dmod = 0;
+  for (int m = 1; m < M; m++) if (Dm[m] > Dm[dmod]) dmod = m;
+  const double J = __dsub_rn(__dsub_rn(W, __dmul_rn((double)a.p.lambda_l, (double)T)),
+                             __dmul_rn(__dmul_rn((double)a.p.lambda_ld, (double)a.levels[l]), (double)Dt));
+  o.corr[rec] = dec_f32(a.gJ[rec]);
+  if (o.corr64) o.corr64[rec] = J;
+  o.lat[rec] = (int)T;
+  for (int bb = 0; bb < B; bb++) o.dem[rec * B + bb] = D[bb];
+  o.dom_model[rec] = (uint8_t)dmod;
+  o.status[rec] = DYPLAN_ST_OK;
+  if (a.extra.dtau) a.extra.dtau[rec] = (int)Dt;
+  if (a.extra.quality) a.extra.quality[rec] = qual;
+}
+
+cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s) {
+  if (a.in.R == 0) return cudaSuccess;
+  k_lstage<<<(unsigned)((a.in.R + 127) / 128), 128, 0, s>>>(a);
+  k_lscore<0><<<grid, 128, 0, s>>>(a);
+  k_lscore<1><<<grid, 128, 0, s>>>(a);
+  const long long nrec = (long long)a.in.R * a.L;
+  k_lemit<<<(unsigned)((nrec + 127) / 128), 128, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace dyplan

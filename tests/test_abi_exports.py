@@ -29,7 +29,8 @@ def test_header_declares_the_three_calls():
     for n in ("dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_create", "dyplan_destroy"):
         assert n in names
     assert "dyplan_switch" in names
-    assert len(names) == 13
+    assert "dyplan_compile_linear" in names
+    assert len(names) == 14
 
 
 def test_library_exports_every_declared_symbol(binding):

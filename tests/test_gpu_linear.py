@@ -1,0 +1,166 @@
+"""-m gpu: dyplan_compile_linear (the paper's objective, Eq.(4)/(5)) against oracle/linear_oracle.c.
+
+Matching rules (the linear-mode twin of tests/parity.py): status equal; the oracle's score of the GPU's chosen plan is
+bit-identical in T and D_tau and within 1e-12 of the GPU's fp64 J and within TOL of its fp32 J; J64(GPU plan) >= J* - TOL;
+identical plan index whenever the oracle's top two are separated by more than TOL.  TOL = 1e-5 * scale with
+scale = sum_n max_k |w| + lambda_l T_max + lambda_ld L D_max: the scorer adds N + 2 fp32 terms of that magnitude
+(error <= (N + 3) 2^-24 scale ~ 1e-6 scale)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2607_02942_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+P0 = dict(lambda_f=0.5, lambda_c=0.1, lambda_l=0.0005, lambda_ld=0.0002, beta=0.5, effort=1.0)
+
+
+@pytest.fixture(scope="module")
+def dy():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2607_02942_b200 import binding
+    ctx = binding.Context(0)
+    yield binding, ctx
+    ctx.close()
+
+
+def f32(p):
+    return {k: float(np.float32(v)) for k, v in p.items()}
+
+
+def run_gpu(dy, batch, cost, params, levels):
+    import torch
+    binding, ctx = dy
+    R, L, B = batch.R, len(levels), batch.B
+    db = binding.make_batch(batch, "cuda:0")
+    out = binding.alloc_bundle(R, L, B, "cuda:0", True)
+    dcost = torch.from_numpy(np.ascontiguousarray(cost, np.float32)).cuda()
+    dtau = torch.full((R * L,), -5, dtype=torch.int32, device="cuda")
+    qual = torch.full((R * L,), -5.0, dtype=torch.float64, device="cuda")
+    ctx.dyplan_compile_linear(db, dcost, params, levels, out, dtau, qual)
+    torch.cuda.synchronize()
+    g = out.host()
+    g["dtau"] = dtau.cpu().numpy()
+    g["quality"] = qual.cpu().numpy()
+    return g, ctx.dyplan_last_stats()
+
+
+def check(lo, batch, cost, params, levels, g, ref):
+    L = len(levels)
+    ch = g["choice"].reshape(-1, 16)
+    same = 0
+    for rec in range(batch.R * L):
+        r, l = divmod(rec, L)
+        assert int(g["status"][rec]) == int(ref["status"][rec]), rec
+        if ref["status"][rec] != 0:
+            assert g["plan_idx"][rec] == np.iinfo(np.uint64).max and g["corr"][rec] == -1.0
+            continue
+        n0, N = int(batch.node_off[r]), batch.n_nodes(r)
+        # scale of the objective's terms
+        scale = params["lambda_l"] * float(ref["T"][rec]) + params["lambda_ld"] * levels[l] * float(ref["Dtau"][rec]) + N * (
+            1.0 + params["beta"] + params["lambda_f"] + params["lambda_c"] * float(np.max(cost)))
+        tol = 1e-5 * max(scale, 1.0)
+        s = lo.score(batch, cost, params, r, levels[l], ch[rec].copy())
+        assert s["status"] == 0
+        assert s["T"] == int(g["lat"][rec]) and s["Dtau"] == int(g["dtau"][rec]), rec
+        assert abs(s["J"] - float(g["corr64"][rec])) <= 1e-12 * max(1.0, abs(s["J"])), rec
+        assert abs(s["J"] - float(g["corr"][rec])) <= tol, rec
+        assert s["J"] >= float(ref["J"][rec]) - tol, (rec, s["J"], ref["J"][rec])
+        assert s["J"] <= float(ref["J"][rec]) + 1e-12 * max(1.0, abs(s["J"]))
+        # canonical index consistent with the choice digits
+        idx, mul = 0, 1
+        for n in range(N):
+            idx += int(ch[rec, n]) * mul
+            mul *= int(batch.opt_off[n0 + n + 1] - batch.opt_off[n0 + n])
+        assert idx == int(g["plan_idx"][rec]) and (ch[rec, N:] == 0xFF).all()
+        # the quality annotation is the product-form C of the chosen plan
+        q = 1.0
+        for n in range(N):
+            o = int(batch.opt_off[n0 + n]) + int(ch[rec, n])
+            q *= 1.0 - float(batch.vuln[n0 + n]) * (1.0 - float(batch.acc[o]))
+        assert abs(q - float(g["quality"][rec])) <= 1e-12
+        if int(g["plan_idx"][rec]) == int(ref["plan_idx"][rec]):
+            same += 1
+        else:
+            run = float(ref["runner_J"][rec])
+            assert not np.isnan(run) and float(ref["J"][rec]) - run <= tol, (rec, ref["J"][rec], run)
+    return same
+
+
+def case(seed, R, nmin, nmax, kmin, kmax, tool_p=0.0):
+    w = wl.random_workload(seed, R=R, nmin=nmin, nmax=nmax, kmin=kmin, kmax=kmax, B=3, M=3, L=1, caps=False, tool_p=tool_p)
+    rng = np.random.default_rng(seed + 1)
+    return w.batch, rng.uniform(0.0, 1.0, size=w.batch.lat_us.size).astype(np.float32)
+
+
+@pytest.mark.parametrize("seed,levels", [(201, [0.0]), (202, [0.0, 1.5, 3.0]), (203, [0.0, 0.5, 1.0, 2.0, 4.0, 8.0, 16.0, 32.0])])
+def test_linear_random_ragged(dy, seed, levels):
+    from oracle import linear as lo
+    batch, cost = case(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=6, tool_p=0.2)
+    p = f32(P0)
+    g, st = run_gpu(dy, batch, cost, p, levels)
+    ref = lo.compile(batch, cost, p, [float(np.float32(x)) for x in levels])
+    same = check(lo, batch, cost, p, [float(np.float32(x)) for x in levels], g, ref)
+    assert same >= 0.9 * batch.R * len(levels)
+    assert st["launches"] == 4
+
+
+def test_linear_cfg1_shaped_requests(dy):
+    # BASELINE.json configs[1] shapes (8 nodes x 8 options) under the paper's objective, three levels as in PAPER.md:299
+    from oracle import linear as lo
+    w = wl.make_config(1, R=3)
+    rng = np.random.default_rng(9)
+    cost = rng.uniform(0.0, 1.0, size=w.batch.lat_us.size).astype(np.float32)
+    p = f32(dict(P0, lambda_l=0.0002, lambda_ld=0.0001))
+    levels = [0.0, 1.5, 3.0]
+    g, st = run_gpu(dy, w.batch, cost, p, levels)
+    assert st["plans"] == 3 * 8**8
+    ref = lo.compile(w.batch, cost, p, levels)
+    check(lo, w.batch, cost, p, levels, g, ref)
+    # raising the level cannot raise the chosen plan's D_tau
+    assert (np.diff(g["dtau"].reshape(3, 3), axis=1) <= 0).all()
+
+
+def test_linear_fig7_example_and_statuses(dy):
+    from oracle import linear as lo
+    from test_linear_pins import fig7_batch
+    b = fig7_batch()
+    cost = np.array([0.3, 0.2, 0.1, 0.15, 0.1], np.float32)
+    p = f32(dict(lambda_f=0.4, lambda_c=0.05, lambda_l=0.01, lambda_ld=0.02, beta=0.0, effort=0.0))
+    g, _ = run_gpu(dy, b, cost, p, [0.0, 1.5, 3.0])
+    ch = g["choice"].reshape(3, 16)
+    assert ch[0, :2].tolist() == [1, 0] and ch[2, :2].tolist() == [2, 1]       # Fig. 7(b): pi(0) then pi(1)
+    assert g["dtau"].tolist()[0] == 17 and g["dtau"].tolist()[2] == 10 and g["lat"].tolist()[0] == 10
+    # malformed and out-of-range requests are isolated
+    batch, cost = case(204, R=8, nmin=2, nmax=5, kmin=2, kmax=4)
+    batch.vuln[int(batch.node_off[1])] = np.nan
+    cost[int(batch.opt_off[int(batch.node_off[3])])] = -1.0
+    a, e = int(batch.opt_off[int(batch.node_off[5])]), int(batch.opt_off[int(batch.node_off[6])])
+    batch.lat_us[a:e] = 3_000_000                                              # duration sum beyond 2^22: TOO_LARGE
+    g, _ = run_gpu(dy, batch, cost, f32(P0), [0.0, 2.0])
+    st = g["status"].reshape(8, 2)
+    assert (st[1] == 2).all() and (st[3] == 2).all() and (st[5] == 3).all()
+    ok = [0, 2, 4, 6, 7]
+    ref = lo.compile(batch.subset(ok), np.concatenate([cost[int(batch.opt_off[int(batch.node_off[r])]): int(batch.opt_off[int(batch.node_off[r + 1])])] for r in ok]), f32(P0), [0.0, 2.0])
+    assert np.array_equal(g["plan_idx"].reshape(8, 2)[ok].reshape(-1), ref["plan_idx"])
+
+
+def test_linear_argument_errors(dy):
+    binding, ctx = dy
+    batch, cost = case(205, R=2, nmin=2, nmax=3, kmin=2, kmax=3)
+    import torch
+    db = binding.make_batch(batch, "cuda:0")
+    out = binding.alloc_bundle(2, 1, 3, "cuda:0", True)
+    dcost = torch.from_numpy(cost).cuda()
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_compile_linear(db, dcost, dict(P0, effort=1.5), [0.0], out)
+    assert e.value.code == binding.ERR_ARG
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_compile_linear(db, dcost, P0, [0.0, -1.0], out)
+    assert e.value.code == binding.ERR_ARG
+    with pytest.raises(binding.DyplanError) as e:
+        ctx.dyplan_compile_linear(db, None, P0, [0.0], out)
+    assert e.value.code == binding.ERR_NULL
