@@ -286,6 +286,116 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
+LINEAR_PARAMS = dict(lambda_f=0.5, lambda_c=0.1, lambda_l=0.0002, lambda_ld=0.0001, beta=0.5, effort=1.0)
+LINEAR_LEVELS = [0.0, 1.5, 3.0]          # the paper's levels
+
+
+def run_linear(args, rank: int, world: int, local_rank: int):
+    """--objective linear: dyplan_compile_linear (the paper's Eq.(4)/(5)) on the configured shape, cost ~ U[0,1]."""
+    import torch
+    import torch.distributed as dist
+    from paper_2607_02942_b200 import binding
+    from paper_2607_02942_b200.multi import max_over_ranks, whole_job_rate
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the dyplan path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    ctx = binding.Context(local_rank)
+    w = make_workload(args.config, rank, args.requests)
+    b = w.batch
+    cost = np.random.default_rng(7 + rank).uniform(0.0, 1.0, size=b.lat_us.size).astype(np.float32)
+    L = len(LINEAR_LEVELS)
+    plans = w.n_plans_total()
+    evals = plans * L
+    stream = torch.cuda.Stream(device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    db = binding.make_batch(b, dev)
+    out = binding.alloc_bundle(b.R, L, b.B, dev, True)
+    dcost = torch.from_numpy(cost).to(dev)
+    sampler = ClockSampler(local_rank)
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            ctx.dyplan_compile_linear(db, dcost, LINEAR_PARAMS, LINEAR_LEVELS, out, stream=stream)
+        stream.synchronize()
+        st = ctx.dyplan_last_stats()
+        assert st["plans"] == plans, (st, plans)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        sampler.start()
+        e0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+        e1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+        for i in range(args.steps):
+            flush.fill_(i & 0xFF)
+            e0[i].record(stream)
+            ctx.dyplan_compile_linear(db, dcost, LINEAR_PARAMS, LINEAR_LEVELS, out, stream=stream)
+            e1[i].record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        tot_ms = sum(a.elapsed_time(c) for a, c in zip(e0, e1))
+    # end to end: pinned host arrays -> device, compile, records -> host, inside the timed region
+    hb = binding.make_batch(b, None)
+    pinned = {k: torch.from_numpy(a.view({np.dtype(np.uint32): np.int32}.get(a.dtype, a.dtype))).pin_memory()
+              for k, a in hb.arrays.items() if a is not None}
+    pcost = torch.from_numpy(cost).pin_memory()
+    h2d = sum(t.numel() * t.element_size() for t in pinned.values()) + pcost.numel() * 4
+    d2h = 0
+    e2e_ms = 0.0
+    for i in range(args.steps + 1):
+        flush.fill_(i & 0xFF)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(stream):
+            for k, t in pinned.items():
+                tgt = db.arrays[k]
+                tgt.view(t.dtype).copy_(t, non_blocking=True) if tgt.dtype != t.dtype else tgt.copy_(t, non_blocking=True)
+            dcost.copy_(pcost, non_blocking=True)
+            ctx.dyplan_compile_linear(db, dcost, LINEAR_PARAMS, LINEAR_LEVELS, out, stream=stream)
+            res = {k: v.to("cpu", non_blocking=False) for k, v in out.arrays.items() if v is not None}
+        stream.synchronize()
+        if i:
+            e2e_ms += 1e3 * (time.perf_counter() - t0)
+        d2h = sum(v.numel() * v.element_size() for v in res.values())
+    tot_ms, e2e_ms = max_over_ranks([tot_ms, e2e_ms], device=dev)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    aops = 2.0 + 5.0 / L      # per (plan, level): FFMA + compare; per plan: add-min (2), two sums, one FFMA
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak = st["sm_count"] * SM_LANES * sm_max * 1e6 / 1e12
+    k_eval_s = evals * args.steps / (tot_ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": whole_job_rate(evals, world, args.steps, tot_ms) / 1e9, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}] shapes ({w.name}) under the paper's linear objective "
+                               f"Eq.(4)/(5), levels {LINEAR_LEVELS}, cost ~ U[0,1]", "requests_per_gpu": b.R,
+                   "plans_per_gpu": plans, "levels": L, "l2": "flushed between timed iterations (256 MiB fill)"},
+        "requests_per_s": world * b.R * args.steps / (tot_ms * 1e-3),
+        "e2e": {"value": world * evals * args.steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps, "api": "dyplan_compile_linear + copies"},
+        "gpu_launches": st["launches"] * args.steps, "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "k_lscore (two passes)", "achieved": k_eval_s * aops / 1e12, "peak": peak,
+                     "unit": "Tinst/s", "frac": k_eval_s * aops / 1e12 / peak, "traffic": None, "ops_per_eval": aops,
+                     "kernel_ms": st["score_ms"]},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import linear as lo
+        sub = w.subset([0])
+        c0 = cost[: sub.batch.lat_us.size]
+        t0 = time.perf_counter()
+        lo.compile(sub.batch, c0, LINEAR_PARAMS, LINEAR_LEVELS)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": sub.n_plans_total() * L / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"request 0 of {b.R}, every plan, all levels ({dt:.1f} s; one request runs on one core)"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -297,12 +407,16 @@ def main():
     ap.add_argument("--cpu-requests", type=int, default=32, help="oracle sample size of the cpu_baseline leg")
     ap.add_argument("--ref-requests", type=int, default=4, help="oracle sample size per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--objective", default="product", choices=["product", "linear"],
+                    help="product: north_star's constrained objective (default); linear: the paper's Eq.(4)/(5)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "dyplan" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.objective == "linear":
+        run_linear(args, rank, world, local_rank)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_dyplan(args, rank, world, local_rank)

@@ -146,12 +146,12 @@ cudaError_t launch_switch(const SwitchArgs& a, cudaStream_t s);
 
 // ---- linear mode (dyplan_linear.cu) ----
 constexpr int kLinHdrWords = 88;                        // LinHdr size in words
-constexpr int kLinBlobWords = kLinHdrWords + 2 * (16 * 16 + 2);   // header + w[slot] + d[slot]
+constexpr int kLinBlobWords = kLinHdrWords + 2 * (16 * 16 + 4);   // header + (w, d)[slot]
 struct LinHdr {
   int32_t status;                 // DYPLAN_ST_OK / _INVALID / _TOO_LARGE
   int32_t n_orig, n_int;          // real nodes, nodes incl. dummies (>= 2)
   int32_t pad0;
-  unsigned long long outer_total; // prod_{i>=2} K_i
+  unsigned long long outer_total; // prod_{i>=3} K_i
   unsigned long long pad1;
   int32_t K[16];                  // options per internal node (1 for dummies)
   uint32_t succ[16];              // successor mask per node (all bits > i)

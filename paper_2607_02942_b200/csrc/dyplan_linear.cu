@@ -23,8 +23,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   const int L = a.L;
   uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
   LinHdr* h = (LinHdr*)blob;
-  float* t_w = (float*)(blob + kLinHdrWords);
-  float* t_d = t_w + (16 * 16 + 2);
+  float2* t_wd = (float2*)(blob + kLinHdrWords);   // (w, d) per slot
   for (int l = 0; l < L; l++) { a.gJ[r * L + l] = INT32_MIN; a.gKey[r * L + l] = ~0ull; }
 
   int st = DYPLAN_ST_OK;
@@ -52,7 +51,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
     }
     if (st == DYPLAN_ST_OK && dsum > (1ull << 22)) st = DYPLAN_ST_TOO_LARGE;
   }
-  h->status = st; h->n_orig = N; h->n_int = N < 2 ? 2 : N; h->pad0 = 0;
+  h->status = st; h->n_orig = N; h->n_int = N < 3 ? 3 : N; h->pad0 = 0;
   if (st != DYPLAN_ST_OK) {
     h->outer_total = 0;
     for (int l = 0; l < L; l++) {
@@ -85,7 +84,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   }
   unsigned long long stride = 1, outer = 1;
   int slot = 0;
-  const int Np = N < 2 ? 2 : N;
+  const int Np = N < 3 ? 3 : N;
   for (int n = 0; n < 16; n++) {
     if (n < N) {
       const int ob = b.opt_off[n0 + n], K = b.opt_off[n0 + n + 1] - ob;
@@ -94,31 +93,36 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
       h->K[n] = K; h->succ[n] = succ[n]; h->optbase[n] = slot; h->stride[n] = stride;
       for (int k = 0; k < K; k++) {
         const double q = (double)b.acc[ob + k];
-        t_w[slot + k] = (float)(rho * q - (double)a.p.lambda_f * v * (1.0 - q) - (double)a.p.lambda_c * (double)a.cost[ob + k]);
-        t_d[slot + k] = (float)b.lat_us[ob + k];
+        t_wd[slot + k] = make_float2((float)(rho * q - (double)a.p.lambda_f * v * (1.0 - q) - (double)a.p.lambda_c * (double)a.cost[ob + k]),
+                                     (float)b.lat_us[ob + k]);
       }
       slot += K;
       stride *= (unsigned long long)K;
-      if (n >= 2) outer *= (unsigned long long)K;
+      if (n >= 3) outer *= (unsigned long long)K;
     } else {
       h->K[n] = 1; h->succ[n] = 0; h->optbase[n] = slot; h->stride[n] = 0;
-      if (n < Np) { t_w[slot] = 0.0f; t_d[slot] = 0.0f; slot += 1; }   // dummy node: one neutral option
+      if (n < Np) { t_wd[slot] = make_float2(0.0f, 0.0f); slot += 1; }   // dummy node: one neutral option
     }
   }
   h->outer_total = outer;
   atomicAdd(a.plans, P);
 }
 
-// One warp per work item (request r, chunk c): outer indices [c*per, (c+1)*per) of the request, split over the lanes.
-template <int PASS>
+// One warp per work item (request r, chunk c): a range of outer indices (digits of the nodes >= 3) of the request, split
+// over the lanes.  Per outer index: digits by div/mod, slack DP of the nodes >= 3 from the last node down
+// (u[i] = min(0, min_succ u[j]) - d: T = -min u); then loops over the options of nodes 2, 1, 0 with one fused step each.
+template <int PASS, int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
 __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
-  const int lane = threadIdx.x & 31;
+  __shared__ __align__(16) uint32_t s_blob[4][kLinBlobWords];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t* sb = s_blob[wid];
   const int L = a.L;
   const uint32_t total = (uint32_t)a.in.R * a.chunks;
-  float cl[DYPLAN_MAX_LEVELS];
+  float cl[LT];
 #pragma unroll
-  for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) cl[l] = l < L ? -(a.p.lambda_ld * a.levels[l]) : 0.0f;
+  for (int l = 0; l < LT; l++) cl[l] = l < L ? -(a.p.lambda_ld * a.levels[l]) : 0.0f;
   const float lam_l = a.p.lambda_l;
+  long long cur_req = -1;
   for (;;) {
     uint32_t item = 0;
     if (lane == 0) item = atomicAdd(&a.counter[PASS], 1u);
@@ -126,71 +130,95 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
     if (item >= total) break;
     const long long r = item / a.chunks;
     const uint32_t c = item % a.chunks;
-    const uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
-    const LinHdr* h = (const LinHdr*)blob;
+    if (r != cur_req) {
+      const uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
+      __syncwarp();
+      for (int i = lane; i < kLinBlobWords; i += 32) sb[i] = __ldg(&blob[i]);
+      __syncwarp();
+      cur_req = r;
+    }
+    const LinHdr* h = (const LinHdr*)sb;
     if (h->status != DYPLAN_ST_OK) continue;
-    const float* t_w = (const float*)(blob + kLinHdrWords);
-    const float* t_d = t_w + (16 * 16 + 2);
-    const unsigned long long outer = h->outer_total;
+    const float2* t_wd = (const float2*)(sb + kLinHdrWords);   // (w, d) per slot
+    const unsigned long long outer = h->outer_total;            // prod_{i>=3} K_i
     const unsigned long long per = (outer + a.chunks - 1) / a.chunks;
     const unsigned long long cb = min((unsigned long long)c * per, outer), ce = min(cb + per, outer);
     const unsigned long long lper = (ce - cb + 31) / 32;
     const unsigned long long ob = min(cb + lane * lper, ce), oe = min(ob + lper, ce);
-    const int Np = h->n_int, K0 = h->K[0], K1 = h->K[1];
-    const uint32_t succ0 = h->succ[0], succ1 = h->succ[1];
-    const bool conn01 = (succ0 >> 1) & 1;
-    const unsigned long long st0 = h->stride[0], st1 = h->stride[1];
-    const int ob1 = h->optbase[1];
+    const int Np = h->n_int, K0 = h->K[0], K1 = h->K[1], K2 = h->K[2];
+    const uint32_t succ0 = h->succ[0], succ1 = h->succ[1], succ2 = h->succ[2];
+    const bool c01 = (succ0 >> 1) & 1, c02 = (succ0 >> 2) & 1, c12 = (succ1 >> 2) & 1;
+    const unsigned long long st0 = h->stride[0], st1 = h->stride[1], st2 = h->stride[2];
+    const int ob1 = h->optbase[1], ob2 = h->optbase[2];
 
-    float best[DYPLAN_MAX_LEVELS], tgt[DYPLAN_MAX_LEVELS];
-    unsigned long long kmin[DYPLAN_MAX_LEVELS];
+    float best[LT], tgt[LT];
+    unsigned long long kmin[LT];
 #pragma unroll
-    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+    for (int l = 0; l < LT; l++) {
       best[l] = -INFINITY; kmin[l] = ~0ull;
-      tgt[l] = (PASS == 1 && l < L) ? dec_f32(__ldcg(&a.gJ[r * L + l])) : 0.0f;
+      tgt[l] = (PASS == 1 && l < L) ? dec_f32(__ldcg(&a.gJ[r * L + l])) : __int_as_float(0x7fc00000);   // NaN never matches
     }
     float u[16];
     for (unsigned long long o = ob; o < oe; o++) {
-      // digits of the nodes >= 2, their slack DP from the last node down (u[i] = min(0, min_succ u[j]) - d: T = -min u)
       unsigned long long t = o, idxo = 0;
       int dig[16];
-      for (int i = 2; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
+      for (int i = 3; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
       float Wp = 0.0f, Dp = 0.0f, Rm = 0.0f;
-      for (int i = Np - 1; i >= 2; --i) {
-        const int slot = h->optbase[i] + dig[i];
+      for (int i = Np - 1; i >= 3; --i) {
+        const float2 wd = t_wd[h->optbase[i] + dig[i]];
         float m = 0.0f;
         for (uint32_t dm = h->succ[i]; dm; dm &= dm - 1) m = fminf(m, u[__ffs(dm) - 1]);
-        const float d = t_d[slot];
-        u[i] = m - d;
+        u[i] = m - wd.y;
         Rm = fminf(Rm, u[i]);
-        Wp += t_w[slot];
-        Dp += d;
+        Wp += wd.x;
+        Dp += wd.y;
       }
-      float u1in = 0.0f, a0in = 0.0f;
-      for (uint32_t dm = succ1; dm; dm &= dm - 1) u1in = fminf(u1in, u[__ffs(dm) - 1]);
-      for (uint32_t dm = succ0 & ~3u; dm; dm &= dm - 1) a0in = fminf(a0in, u[__ffs(dm) - 1]);
-      for (int k1 = 0; k1 < K1; k1++) {
-        const float d1 = t_d[ob1 + k1];
-        const float u1 = u1in - d1;
-        const float R1 = fminf(Rm, u1);
-        const float W1 = Wp + t_w[ob1 + k1];
-        const float D1 = Dp + d1;
-        const float ap = conn01 ? fminf(a0in, u1) : a0in;
-        const unsigned long long idx1 = idxo + (unsigned long long)k1 * st1;
-        for (int k0 = 0; k0 < K0; k0++) {
-          const float d0 = t_d[k0];
-          const float m = fminf(R1, ap - d0);          // least slack = -T
-          const float W0 = W1 + t_w[k0];
-          const float D0 = D1 + d0;
-          const float Jb = fmaf(lam_l, m, W0);         // W - lambda_l T
+      float u2in = 0.0f, u1in3 = 0.0f, a0in3 = 0.0f;
+      for (uint32_t dm = succ2; dm; dm &= dm - 1) u2in = fminf(u2in, u[__ffs(dm) - 1]);
+      for (uint32_t dm = succ1 & ~7u; dm; dm &= dm - 1) u1in3 = fminf(u1in3, u[__ffs(dm) - 1]);
+      for (uint32_t dm = succ0 & ~7u; dm; dm &= dm - 1) a0in3 = fminf(a0in3, u[__ffs(dm) - 1]);
+      for (int k2 = 0; k2 < K2; k2++) {
+        const float2 wd2 = t_wd[ob2 + k2];
+        const float u2 = u2in - wd2.y;
+        const float R2 = fminf(Rm, u2);
+        const float W2 = Wp + wd2.x, D2 = Dp + wd2.y;
+        const float u1in = c12 ? fminf(u1in3, u2) : u1in3;
+        const float a0in = c02 ? fminf(a0in3, u2) : a0in3;
+        const unsigned long long idx2 = idxo + (unsigned long long)k2 * st2;
+        for (int k1 = 0; k1 < K1; k1++) {
+          const float2 wd1 = t_wd[ob1 + k1];
+          const float u1 = u1in - wd1.y;
+          const float R1 = fminf(R2, u1);
+          const float W1 = W2 + wd1.x, D1 = D2 + wd1.y;
+          const float ap = c01 ? fminf(a0in, u1) : a0in;
+          const unsigned long long idx1 = idx2 + (unsigned long long)k1 * st1;
+          bool hit = false;
+#pragma unroll 4
+          for (int k0 = 0; k0 < K0; k0++) {
+            const float2 wd0 = t_wd[k0];
+            const float m = fminf(R1, ap - wd0.y);        // least slack = -T
+            const float D0 = D1 + wd0.y;
+            const float Jb = fmaf(lam_l, m, W1 + wd0.x);  // W - lambda_l T
 #pragma unroll
-          for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
-            if (l < L) {
-              const float J = fmaf(cl[l], D0, Jb);     // ... - lambda_ld L D_tau
+            for (int l = 0; l < LT; l++) {
+              const float J = fmaf(cl[l], D0, Jb);        // ... - lambda_ld L D_tau
               if (PASS == 0) best[l] = fmaxf(best[l], J);
-              else if (J == tgt[l]) {
-                const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
-                kmin[l] = key < kmin[l] ? key : kmin[l];
+              else hit |= (J == tgt[l]);
+            }
+          }
+          if (PASS == 1 && hit) {
+            // rare: some plan of this group attains a level's maximum -- walk the group again for (T, idx)
+            for (int k0 = 0; k0 < K0; k0++) {
+              const float2 wd0 = t_wd[k0];
+              const float m = fminf(R1, ap - wd0.y);
+              const float D0 = D1 + wd0.y;
+              const float Jb = fmaf(lam_l, m, W1 + wd0.x);
+#pragma unroll
+              for (int l = 0; l < LT; l++) {
+                if (l < L && fmaf(cl[l], D0, Jb) == tgt[l]) {
+                  const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
+                  kmin[l] = key < kmin[l] ? key : kmin[l];
+                }
               }
             }
           }
@@ -198,7 +226,7 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
       }
     }
 #pragma unroll
-    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+    for (int l = 0; l < LT; l++) {
       if (l < L) {
         if (PASS == 0) {
           float v = best[l];
@@ -281,8 +309,12 @@ __global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
 cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s) {
   if (a.in.R == 0) return cudaSuccess;
   k_lstage<<<(unsigned)((a.in.R + 127) / 128), 128, 0, s>>>(a);
-  k_lscore<0><<<grid, 128, 0, s>>>(a);
-  k_lscore<1><<<grid, 128, 0, s>>>(a);
+  switch (level_class(a.L)) {
+#define DYPLAN_LCASE(LT_) case LT_: k_lscore<0, LT_><<<grid, 128, 0, s>>>(a); k_lscore<1, LT_><<<grid, 128, 0, s>>>(a); break;
+    DYPLAN_LCASE(1) DYPLAN_LCASE(2) DYPLAN_LCASE(3) DYPLAN_LCASE(4) DYPLAN_LCASE(6)
+    default: k_lscore<0, 8><<<grid, 128, 0, s>>>(a); k_lscore<1, 8><<<grid, 128, 0, s>>>(a); break;
+#undef DYPLAN_LCASE
+  }
   const long long nrec = (long long)a.in.R * a.L;
   k_lemit<<<(unsigned)((nrec + 127) / 128), 128, 0, s>>>(a);
   return cudaGetLastError();
