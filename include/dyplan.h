@@ -165,6 +165,40 @@ DYPLAN_API int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dypl
                   const uint32_t* dispatched_mask /*[R]*/, int32_t* cur_variant /*[R] in/out*/,
                   uint8_t* active_choice /*[R*16] in/out*/, uint8_t* switched /*[R] out*/, void* stream);
 
+/* Coefficient construction, Algorithm 1 l.1-8 and Eq.(2): bind the offline
+ * profiles to the candidate implementations of every node, producing the per-node / per-option arrays the compile
+ * calls read.  For node n with skill tag s, role rho and fan-in f (the number of predecessor bits), and option k with
+ * model m, backend d and verification policy p:
+ *     vuln[n]   = psi[role][s][min(f, F-1)]                                       v_n = Psi(role, skill, fan-in)
+ *     acc[k]    = quality[s][m][p]                                                q = Q^(s, m, p),
+ *     lat_us[k] = rint( 1e6 * sum_a max_j tokens[s][m][p][a][j] / theta_dec[m][d] + tau_pre_us[m][d] )     Eq.(2)
+ *                 ("serial stage durations add, a parallel stage contributes its longest nominal call")
+ *     cost[k]   = ( sum_a sum_j tokens[s][m][p][a][j] ) / token_norm              "normalized token count across all base
+ *                 and verification calls, including those that execute in parallel"
+ * tokens = 0 marks an absent call; stage 0 is base generation.  Gated policies carry their expected demand in the
+ * profile (App. A).  theta_dec is in tokens per second at the calibration point b_0.  An index out of
+ * range (skill, role, model, backend, policy) or a non-positive theta_dec gives vuln = NaN / acc = NaN / lat_us = -1,
+ * which the compile calls report as INVALID for that request.  The arrays of `prof` and every other pointer are DEVICE
+ * pointers; `prof` itself is a HOST struct.  demand[k] (optional output, may be NULL) = the option's total token count
+ * rounded to int32, the per-model demand annotation of PAPER.md:211. */
+typedef struct {
+  int32_t S, M, P, D;      /* skill classes, models, verification policies, backends                     */
+  int32_t A, J;            /* stages per policy (incl. base generation), parallel calls per stage        */
+  int32_t ROLES, F;        /* structural roles, fan-in buckets                                           */
+  const float* quality;    /* [S*M*P]                                                                    */
+  const float* tokens;     /* [S*M*P*A*J] profiled output-token count of call j in stage a               */
+  const float* theta_dec;  /* [M*D] calibrated decode rate, tokens/s                                     */
+  const float* tau_pre_us; /* [M*D] aggregate prefill-latency correction, microseconds                   */
+  const float* psi;        /* [ROLES*S*F]                                                                */
+  float token_norm;        /* > 0                                                                        */
+} dyplan_profiles;
+
+DYPLAN_API int dyplan_bind(dyplan_ctx* ctx, const dyplan_profiles* prof, int32_t NN, int32_t KK, const int32_t* opt_off /*[NN+1]*/,
+                const uint32_t* pred_mask /*[NN]*/, const uint8_t* skill /*[NN]*/, const uint8_t* role /*[NN]*/,
+                const uint8_t* model /*[KK]*/, const uint8_t* backend /*[KK]*/, const uint8_t* policy /*[KK]*/,
+                float* vuln /*[NN] out*/, float* acc /*[KK] out*/, int32_t* lat_us /*[KK] out*/, float* cost /*[KK] out*/,
+                int32_t* demand /*[KK] out or NULL*/, void* stream);
+
 /* The paper's own objective ("linear mode", Eq.(4)/(5)) over the same plan space, by exhaustive
  * enumeration: for every level L_k maximise
  *     J_L(pi) = sum_n [ rho(n) q - lambda_f v_n (1 - q) - lambda_c c ](n, k_n)  -  lambda_l T(pi)  -  lambda_ld L D_tau(pi)

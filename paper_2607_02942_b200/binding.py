@@ -26,7 +26,7 @@ FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
 EXPORTS = (
-    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear",
+    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_bind",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
 )
@@ -63,6 +63,12 @@ class CLinearExtra(C.Structure):
     _fields_ = [("dtau", C.c_void_p), ("quality", C.c_void_p)]
 
 
+class CProfiles(C.Structure):
+    _fields_ = [("S", C.c_int32), ("M", C.c_int32), ("P", C.c_int32), ("D", C.c_int32), ("A", C.c_int32), ("J", C.c_int32),
+                ("ROLES", C.c_int32), ("F", C.c_int32), ("quality", C.c_void_p), ("tokens", C.c_void_p),
+                ("theta_dec", C.c_void_p), ("tau_pre_us", C.c_void_p), ("psi", C.c_void_p), ("token_norm", C.c_float)]
+
+
 class CStats(C.Structure):
     _fields_ = [("plans", C.c_uint64), ("evals", C.c_uint64), ("work_items", C.c_uint64), ("slow_steps", C.c_uint64),
                 ("fast_requests", C.c_uint64), ("launches", C.c_int32), ("sm_count", C.c_int32), ("score_ms", C.c_float)]
@@ -87,6 +93,7 @@ def lib():
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
         l.dyplan_compile_linear.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp]
+        l.dyplan_bind.argtypes = [vp, C.POINTER(CProfiles), i32, i32] + [vp] * 13
         l.dyplan_switch.argtypes = [vp, pb, po, i32, C.POINTER(CSwitchParams), vp, vp, vp, vp, vp, vp, vp]
         l.dyplan_compile_host.argtypes = [vp, pb, i32, vp, po, vp, pu64, pu64]
         l.dyplan_replan_host.argtypes = [vp, pb, vp, vp, vp, u32, po, vp, pu64, pu64]
@@ -280,6 +287,14 @@ class Context:
         self._check(lib().dyplan_compile_linear(self._h, C.byref(batch.cstruct), _ptr(cost), C.byref(p), int(lv.size),
                                                 lv.ctypes.data_as(C.c_void_p), C.byref(out.cstruct), C.byref(ex),
                                                 _stream_ptr(stream)))
+
+    def dyplan_bind(self, dims: dict, quality, tokens, theta_dec, tau_pre_us, psi, token_norm: float, NN: int, KK: int,
+                    opt_off, pred_mask, skill, role, model, backend, policy, vuln, acc, lat_us, cost, demand=None, stream=None):
+        p = CProfiles(dims["S"], dims["M"], dims["P"], dims["D"], dims["A"], dims["J"], dims["ROLES"], dims["F"],
+                      _ptr(quality), _ptr(tokens), _ptr(theta_dec), _ptr(tau_pre_us), _ptr(psi), float(token_norm))
+        self._check(lib().dyplan_bind(self._h, C.byref(p), NN, KK, _ptr(opt_off), _ptr(pred_mask), _ptr(skill), _ptr(role),
+                                      _ptr(model), _ptr(backend), _ptr(policy), _ptr(vuln), _ptr(acc), _ptr(lat_us),
+                                      _ptr(cost), _ptr(demand), _stream_ptr(stream)))
 
     def dyplan_switch(self, batch: Buffers, bundle: Buffers, L: int, params: dict, model_load, since_switch,
                       dispatched_mask, cur_variant, active_choice, switched, stream=None):

@@ -296,6 +296,33 @@ int dyplan_switch(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* 
   return DYPLAN_OK;
 }
 
+int dyplan_bind(dyplan_ctx* ctx, const dyplan_profiles* prof, int32_t NN, int32_t KK, const int32_t* opt_off, const uint32_t* pred_mask,
+                const uint8_t* skill, const uint8_t* role, const uint8_t* model, const uint8_t* backend, const uint8_t* policy,
+                float* vuln, float* acc, int32_t* lat_us, float* cost, int32_t* demand, void* stream) {
+  if (!ctx || !prof) return DYPLAN_ERR_NULL;
+  if (NN < 0 || KK < 0) return DYPLAN_ERR_LIMIT;
+  if (prof->S < 1 || prof->M < 1 || prof->P < 1 || prof->D < 1 || prof->A < 1 || prof->J < 1 || prof->ROLES < 1 || prof->F < 1 ||
+      prof->S > 256 || prof->M > 256 || prof->P > 256 || prof->D > 256 || prof->ROLES > 256)
+    return DYPLAN_ERR_LIMIT;
+  if (!(prof->token_norm > 0.0f)) return DYPLAN_ERR_ARG;
+  ctx->last_launches = 0;
+  ctx->have_events = false;
+  ctx->last_stream = (cudaStream_t)stream;
+  if (NN == 0) return DYPLAN_OK;
+  if (!prof->quality || !prof->tokens || !prof->theta_dec || !prof->tau_pre_us || !prof->psi || !opt_off || !pred_mask || !skill ||
+      !role || !vuln || (KK > 0 && (!model || !backend || !policy || !acc || !lat_us || !cost)))
+    return DYPLAN_ERR_NULL;
+  CK(cudaSetDevice(ctx->device));
+  BindArgs a;
+  memset(&a, 0, sizeof(a));
+  a.prof = *prof; a.NN = NN; a.KK = KK; a.opt_off = opt_off; a.pred_mask = pred_mask; a.skill = skill; a.role = role;
+  a.model = model; a.backend = backend; a.policy = policy; a.vuln = vuln; a.acc = acc; a.lat_us = lat_us; a.cost = cost;
+  a.demand = demand;
+  CK(launch_bind(a, (cudaStream_t)stream));
+  ctx->last_launches = 1;
+  return DYPLAN_OK;
+}
+
 int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* cost, const dyplan_linear_params* params, int32_t L,
                           const float* levels, dyplan_bundle* out, const dyplan_linear_extra* extra, void* stream) {
   if (!ctx) return DYPLAN_ERR_NULL;

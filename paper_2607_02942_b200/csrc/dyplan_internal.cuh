@@ -144,6 +144,16 @@ struct SwitchArgs {
 };
 cudaError_t launch_switch(const SwitchArgs& a, cudaStream_t s);
 
+// ---- coefficient construction (dyplan_bind.cu) ----
+struct BindArgs {
+  dyplan_profiles prof;
+  int32_t NN, KK;
+  const int32_t* opt_off; const uint32_t* pred_mask; const uint8_t* skill; const uint8_t* role;
+  const uint8_t* model; const uint8_t* backend; const uint8_t* policy;
+  float* vuln; float* acc; int32_t* lat_us; float* cost; int32_t* demand;
+};
+cudaError_t launch_bind(const BindArgs& a, cudaStream_t s);
+
 // ---- linear mode (dyplan_linear.cu) ----
 constexpr int kLinHdrWords = 88;                        // LinHdr size in words
 constexpr int kLinBlobWords = kLinHdrWords + 2 * (16 * 16 + 4);   // header + (w, d)[slot]

@@ -30,7 +30,8 @@ def test_header_declares_the_three_calls():
         assert n in names
     assert "dyplan_switch" in names
     assert "dyplan_compile_linear" in names
-    assert len(names) == 14
+    assert "dyplan_bind" in names
+    assert len(names) == 15
 
 
 def test_library_exports_every_declared_symbol(binding):
