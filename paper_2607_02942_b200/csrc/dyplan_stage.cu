@@ -460,6 +460,12 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   unsigned long long pif = (total_f + tgt - 1) / tgt;
   need = (total_f + budget - 1) / budget;
   if (need > pif) pif = need;
+  // small calls: an item should carry at least 8 outer indices per lane (its fixed cost is a few thousand instructions)
+  // unless that would leave resident warps without work (target_items_f = 24 items per resident warp)
+  const unsigned long long warps = tgt / 24 ? tgt / 24 : 1;
+  unsigned long long floor_f = (total_f + warps - 1) / warps;
+  floor_f = floor_f > 256 ? 256 : floor_f;
+  if (floor_f > pif) pif = floor_f;
   pif = ((pif + 31) / 32) * 32;
   if (pif < 32) pif = 32;
   uint32_t cw = 0, cf = 0;
