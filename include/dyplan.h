@@ -107,9 +107,19 @@ typedef struct {
   uint8_t* status;    /* [R*L]    DYPLAN_ST_*                                                                 */
 } dyplan_bundle;
 
+/* Context flags (dyplan_set_flags; default 0 = every option of every node is enumerated).
+ * DYPLAN_PRUNE_DOMINATED: before enumerating, drop every option that another option of the same node dominates -- at
+ *   least as good a factor f, every level's duration no longer, with caps the same backend and no more demand, and
+ *   strictly preferred (f larger, or f equal and a lower option index).  Exact: a dropped option is in no best plan under
+ *   the fixed order, so results are those of the full enumeration (parity-tested against the unpruned oracle); what
+ *   changes is dyplan_stats.plans, which then counts the plans of the pruned space, and the 2^40 limit, which applies
+ *   to the pruned space.  Applies to requests the fp32 scorer takes; others are enumerated in full. */
+#define DYPLAN_PRUNE_DOMINATED 1u
+
 /* Create / destroy a context on CUDA device `device_ordinal`.  Fails (DYPLAN_ERR_CUDA) without a device. */
 DYPLAN_API int dyplan_create(dyplan_ctx** out, int device_ordinal);
 DYPLAN_API int dyplan_destroy(dyplan_ctx* ctx);
+DYPLAN_API int dyplan_set_flags(dyplan_ctx* ctx, uint32_t flags); /* DYPLAN_ERR_ARG on unknown bits */
 
 /* Algorithm 1 l.10-15 by exhaustive enumeration: best plan per (request, level).
  * mult_pm: [L*B] per-mille latency multipliers >= 0 per (level, backend) -- device pointer (host in *_host). */

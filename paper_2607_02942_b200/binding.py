@@ -26,7 +26,7 @@ FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
 EXPORTS = (
-    "dyplan_create", "dyplan_destroy", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_bind",
+    "dyplan_create", "dyplan_destroy", "dyplan_set_flags", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_bind",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
 )
@@ -48,6 +48,9 @@ class CBatch(C.Structure):
 class CBundle(C.Structure):
     _fields_ = [("plan_idx", C.c_void_p), ("choice", C.c_void_p), ("corr", C.c_void_p), ("corr64", C.c_void_p),
                 ("lat", C.c_void_p), ("dem", C.c_void_p), ("dom_model", C.c_void_p), ("status", C.c_void_p)]
+
+
+PRUNE_DOMINATED = 1
 
 
 class CSwitchParams(C.Structure):
@@ -89,6 +92,7 @@ def lib():
         pb, po, pu64 = C.POINTER(CBatch), C.POINTER(CBundle), C.POINTER(C.c_uint64)
         l.dyplan_create.argtypes = [C.POINTER(vp), C.c_int]
         l.dyplan_destroy.argtypes = [vp]
+        l.dyplan_set_flags.argtypes = [vp, u32]
         l.dyplan_compile.argtypes = [vp, pb, i32, vp, po, vp]
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
@@ -295,6 +299,9 @@ class Context:
         self._check(lib().dyplan_bind(self._h, C.byref(p), NN, KK, _ptr(opt_off), _ptr(pred_mask), _ptr(skill), _ptr(role),
                                       _ptr(model), _ptr(backend), _ptr(policy), _ptr(vuln), _ptr(acc), _ptr(lat_us),
                                       _ptr(cost), _ptr(demand), _stream_ptr(stream)))
+
+    def dyplan_set_flags(self, flags: int):
+        self._check(lib().dyplan_set_flags(self._h, int(flags)))
 
     def dyplan_switch(self, batch: Buffers, bundle: Buffers, L: int, params: dict, model_load, since_switch,
                       dispatched_mask, cur_variant, active_choice, switched, stream=None):

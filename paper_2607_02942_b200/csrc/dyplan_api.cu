@@ -65,6 +65,7 @@ struct dyplan_ctx {
   DevBuf blob, item_off, done, gthr, partial, state;   // item_off holds both classes' offset arrays
   DevBuf lin_blob, lin_gj, lin_gkey, lin_misc;          // linear mode
   bool last_linear = false;
+  uint32_t flags = 0;
   // staging for the *_host calls: one device arena, one pinned-or-not host side is the caller's
   DevBuf arena;
   // occupancy cache [L-1][nb index]
@@ -134,6 +135,13 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
   }
   for (int i = 0; i < 8; i++) { for (int j = 0; j < 4; j++) ctx->occ[i][j] = 0; ctx->focc[i] = 0; }
   *out = ctx;
+  return DYPLAN_OK;
+}
+
+int dyplan_set_flags(dyplan_ctx* ctx, uint32_t flags) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  if (flags & ~DYPLAN_PRUNE_DOMINATED) return DYPLAN_ERR_ARG;
+  ctx->flags = flags;
   return DYPLAN_OK;
 }
 
@@ -217,7 +225,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   CallArgs a;
   memset(&a, 0, sizeof(a));
   a.in = *in; a.out = *out; a.L = L; a.mult = mult; a.dispatched = dispatched; a.fixed_choice = fixed_choice;
-  a.flags = flags; a.is_replan = is_replan ? 1 : 0;
+  a.flags = flags; a.is_replan = is_replan ? 1 : 0; a.ctx_flags = ctx->flags;
   a.blob = (uint32_t*)ctx->blob.p; a.item_off = (uint32_t*)ctx->item_off.p; a.item_off_f = a.item_off + (R + 1);
   a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f;
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;

@@ -97,6 +97,7 @@ struct CallArgs {                   // passed by value to the kernels
   const uint32_t* dispatched;       // replan only
   const uint8_t* fixed_choice;      // replan only
   uint32_t flags;
+  uint32_t ctx_flags;               // DYPLAN_PRUNE_DOMINATED (dyplan_set_flags)
   int32_t is_replan;
   // scratch
   uint32_t* blob;                   // staged requests

@@ -23,6 +23,37 @@ __device__ __forceinline__ long long scaled(int tau, int mult) { return ((long l
 // f = 1 - v (1 - a) in fp64 without contraction (f = v * r^, r^ = 1 - q)
 __device__ __forceinline__ double factor64(float v, float a) { return __dsub_rn(1.0, __dmul_rn((double)v, __dsub_rn(1.0, (double)a))); }
 
+// index of the k-th set bit of m (k < popcount(m))
+__device__ __forceinline__ int nth_set_bit(uint32_t m, int k) {
+  for (int i = 0; i < k; i++) m &= m - 1;
+  return __ffs(m) - 1;
+}
+
+// Exact per-node dominance pruning: option x of a node can be dropped when another
+// option y of the same node is at least as good in every quantity the objective reads -- factor f (as the scorer's
+// fp32 value), every level's scaled duration, and with caps the same backend and no more demand -- and is strictly
+// preferred by order 7 (f larger, or f equal and a lower option index).  Swapping x for y in any plan keeps it feasible
+// (durations enter T monotonically) and makes it strictly better, so no dropped option is in any best plan.
+__device__ uint32_t dominance_keep(const dyplan_batch& b, int o0, int K, float v, const int* mult, int L, int B, bool has_caps) {
+  uint32_t keep = K >= 32 ? 0xffffffffu : ((1u << K) - 1u);
+  for (int x = 0; x < K; x++) {
+    const int ox = o0 + x;
+    const float fx = (float)factor64(v, b.acc[ox]);
+    for (int y = 0; y < K; y++) {
+      if (y == x) continue;
+      const int oy = o0 + y;
+      if (has_caps && (b.backend[oy] != b.backend[ox] || b.demand[oy] > b.demand[ox])) continue;
+      const float fy = (float)factor64(v, b.acc[oy]);
+      if (!(fy > fx || (fy == fx && y < x))) continue;
+      bool ok = true;
+      for (int l = 0; l < L && ok; l++)
+        ok = scaled(b.lat_us[oy], mult[l * B + b.backend[oy]]) <= scaled(b.lat_us[ox], mult[l * B + b.backend[ox]]);
+      if (ok) { keep &= ~(1u << x); break; }
+    }
+  }
+  return keep;
+}
+
 // One warp per request.
 __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   const int lane = threadIdx.x & 31;
@@ -131,15 +162,6 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     bad = __any_sync(0xffffffffu, bad);
     if (bad) st = DYPLAN_ST_INVALID;
   }
-  unsigned long long P = 1;
-  if (st == DYPLAN_ST_OK) {
-#pragma unroll
-    for (int n = 0; n < 16; n++)
-      if (n < N && !((fmask >> n) & 1) && st == DYPLAN_ST_OK) {
-        P *= (unsigned long long)K[n];
-        if (P > (1ull << DYPLAN_MAX_PLANS_LOG2)) st = DYPLAN_ST_TOO_LARGE;
-      }
-  }
   if (st != DYPLAN_ST_OK) {
     if (lane == 0) { h->status = st; h->outer_total = 0; h->nslots_pad = 0; h->K0 = 1; h->K1 = 1; }
     if (lane < L) write_sentinel(a.out, r * L + lane, B, st);
@@ -163,7 +185,6 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   for (int n = 0; n < 16; n++) if (n == e) { myK = K[n]; myo0 = o0[n]; mystride = stride[n]; }
   const bool fixed = e >= 0 && ((fmask >> e) & 1);
   const int fk = fixed ? a.fixed_choice[n0 + e] : 0;
-  const int Kp = (e < 0 || fixed) ? 1 : myK;
   uint32_t deps = 0;
   if (e >= 0) {
     if (!orient) {
@@ -173,60 +194,84 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       for (int p = 0; p < e; p++) if ((pm >> p) & 1) deps |= 1u << (N - 1 - p);
     }
   }
-  const int K0r = __shfl_sync(0xffffffffu, Kp, 0), K1r = __shfl_sync(0xffffffffu, Kp, 1);
 
   // ---- scorer class: the fp32 scorer takes a request when every slack and demand sum is an exact
   // fp32 integer, node 0's options fit its backend-grouped slot layout and the tables fit its shared-memory window ----
   const int Lp = level_class(L);
   const bool has_caps = b.cap != nullptr;
   const int nbc = !has_caps ? 0 : (B <= 2 ? 2 : (B == 3 ? 3 : (B == 4 ? 4 : 8)));
-  // node 0's candidate options: its K options, or the pinned one
+  const bool fast_pre = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)) && min_c >= 1e-30;
+  // options kept per node: all of them, or (opt-in, fast class only) the ones no other option dominates
+  const uint32_t keep_full = (e >= 0 && !fixed) ? (myK >= 32 ? 0xffffffffu : ((1u << myK) - 1u)) : 1u;
+  uint32_t keep = keep_full;
+  bool pruned = (a.ctx_flags & DYPLAN_PRUNE_DOMINATED) && fast_pre;
+  if (pruned && e >= 0 && !fixed && myK > 1) keep = dominance_keep(b, myo0, myK, b.vuln[n0 + e], mult, L, B, has_caps);
   const int e0 = __shfl_sync(0xffffffffu, e, 0), K0all = __shfl_sync(0xffffffffu, myK, 0), o00 = __shfl_sync(0xffffffffu, myo0, 0);
   const int fixed0 = __shfl_sync(0xffffffffu, (int)fixed, 0), fk0 = __shfl_sync(0xffffffffu, fk, 0);
-  int G = 0;
-  if (nbc && e0 >= 0) {
-    int cnt[8];
+  int Kp = 1, K0r = 1, K1r = 1, G = 0, K0p = 2, width = 0, optbase = 0, nslots = 0, nslots_pad = 0, blob_words = 0;
+  bool fast = false;
+  for (int attempt = 0; attempt < 2; attempt++) {
+    Kp = (e < 0 || fixed) ? 1 : __popc(keep);
+    K0r = __shfl_sync(0xffffffffu, Kp, 0);
+    K1r = __shfl_sync(0xffffffffu, Kp, 1);
+    const uint32_t keep0 = __shfl_sync(0xffffffffu, keep, 0);
+    // node 0's candidate options: its kept options, or the pinned one
+    G = 0;
+    if (nbc && e0 >= 0) {
+      int cnt[8];
 #pragma unroll
-    for (int i = 0; i < 8; i++) cnt[i] = 0;
-    for (int k = 0; k < K0all; k++) {
-      if (fixed0 && k != fk0) continue;
-      const int be = (fixed0 && residual) ? 0 : b.backend[o00 + k];
+      for (int i = 0; i < 8; i++) cnt[i] = 0;
+      for (int k = 0; k < K0all; k++) {
+        if (fixed0 ? (k != fk0) : !((keep0 >> k) & 1)) continue;
+        const int be = (fixed0 && residual) ? 0 : b.backend[o00 + k];
 #pragma unroll
-      for (int i = 0; i < 8; i++) cnt[i] += (be == i);
-    }
+        for (int i = 0; i < 8; i++) cnt[i] += (be == i);
+      }
 #pragma unroll
-    for (int i = 0; i < 8; i++) G = cnt[i] > G ? cnt[i] : G;
-  } else if (nbc) G = 1;
-  int K0p = k0_class(K0r);
-  bool fast = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)) && min_c >= 1e-30;
-  if (nbc) {
-    // allowed group sizes per class: nbc*G in {2,4,6,8,12,16}
-    int Gp = 0;
-    if (nbc == 2) Gp = G <= 4 ? (G < 1 ? 1 : G) : (G <= 6 ? 6 : (G <= 8 ? 8 : 0));
-    else if (nbc == 3) Gp = G <= 2 ? 2 : (G <= 4 ? 4 : 0);
-    else if (nbc == 4) Gp = G <= 2 ? (G < 1 ? 1 : G) : (G <= 4 ? 4 : 0);
-    else Gp = G <= 1 ? 1 : (G <= 2 ? 2 : 0);
-    if (Gp == 0) fast = false; else if (fast) { G = Gp; K0p = nbc * Gp; }
-  }
-  int width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
-  int optbase = width;   // inclusive scan over lanes -> exclusive
-#pragma unroll
-  for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
-  int nslots = __shfl_sync(0xffffffffu, optbase, 31);
-  optbase -= width;
-  int nslots_pad = (nslots + 3) & ~3;
-  int blob_words = kHdrWords + nslots_pad * (Lp + 5) + (nbc ? 128 : 0);
-  if (fast && (blob_words > kFastBlobWords || (size_t)blob_words > blob_stride)) {
-    // tables too large for the fp32 scorer's window: fall back to the wide class (recompute the plain layout)
-    fast = false;
+      for (int i = 0; i < 8; i++) G = cnt[i] > G ? cnt[i] : G;
+    } else if (nbc) G = 1;
     K0p = k0_class(K0r);
-    width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
-    optbase = width;
+    fast = fast_pre;
+    if (nbc) {
+      // allowed group sizes per class: nbc*G in {2,4,6,8,12,16}
+      int Gp = 0;
+      if (nbc == 2) Gp = G <= 4 ? (G < 1 ? 1 : G) : (G <= 6 ? 6 : (G <= 8 ? 8 : 0));
+      else if (nbc == 3) Gp = G <= 2 ? 2 : (G <= 4 ? 4 : 0);
+      else if (nbc == 4) Gp = G <= 2 ? (G < 1 ? 1 : G) : (G <= 4 ? 4 : 0);
+      else Gp = G <= 1 ? 1 : (G <= 2 ? 2 : 0);
+      if (Gp == 0) fast = false; else if (fast) { G = Gp; K0p = nbc * Gp; }
+    }
+    for (int lay = 0; lay < 2; lay++) {
+      width = (lane == 0) ? K0p : (lane < Np ? Kp : 0);
+      optbase = width;   // inclusive scan over lanes -> exclusive
 #pragma unroll
-    for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
-    nslots = __shfl_sync(0xffffffffu, optbase, 31);
-    optbase -= width;
-    nslots_pad = (nslots + 3) & ~3;
+      for (int off = 1; off < 32; off <<= 1) { int t = __shfl_up_sync(0xffffffffu, optbase, off); if (lane >= off) optbase += t; }
+      nslots = __shfl_sync(0xffffffffu, optbase, 31);
+      optbase -= width;
+      nslots_pad = (nslots + 3) & ~3;
+      blob_words = kHdrWords + nslots_pad * (Lp + 5) + (nbc ? 128 : 0);
+      if (!(fast && (blob_words > kFastBlobWords || (size_t)blob_words > blob_stride))) break;
+      // tables too large for the fp32 scorer's window: fall back to the wide class (lay out again, plain inner radix)
+      fast = false;
+      K0p = k0_class(K0r);
+    }
+    if (fast || !pruned) break;
+    keep = keep_full;   // pruned, but the request does not fit the fp32 scorer: the int32 scorer enumerates every option
+    pruned = false;
+  }
+  // ---- size of the space to enumerate (after pruning, when it applies) ----
+  {
+    unsigned long long P = 1;
+    bool too_large = false;
+    for (int i = 0; i < Np; i++) {
+      const unsigned long long k = (unsigned long long)__shfl_sync(0xffffffffu, Kp, i);
+      if (P > ((1ull << DYPLAN_MAX_PLANS_LOG2) / k)) too_large = true; else P *= k;
+    }
+    if (too_large) {
+      if (lane == 0) { h->status = DYPLAN_ST_TOO_LARGE; h->outer_total = 0; h->nslots_pad = 0; h->K0 = 1; h->K1 = 1; }
+      if (lane < L) write_sentinel(a.out, r * L + lane, B, DYPLAN_ST_TOO_LARGE);
+      return;
+    }
   }
   unsigned long long outer = (lane >= 2 && lane < Np) ? (unsigned long long)Kp : 1ull;
   unsigned long long base = fixed ? (unsigned long long)fk * mystride : 0ull;
@@ -285,26 +330,31 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       if (s >= ob && s < ob + w) { node = i; k = s - ob; }
     }
     int ne = -1, nK = 1, no0 = 0, nfix = 0, nfk = 0;
+    uint32_t nkeep = 1u;
     unsigned long long nstride = 0;
     for (int i = 0; i < Np; i++) {
       const int ee = __shfl_sync(0xffffffffu, e, i), kk = __shfl_sync(0xffffffffu, myK, i), oo = __shfl_sync(0xffffffffu, myo0, i);
       const int ff = __shfl_sync(0xffffffffu, (int)fixed, i), fkk = __shfl_sync(0xffffffffu, fk, i);
+      const uint32_t kp = __shfl_sync(0xffffffffu, keep, i);
       const unsigned long long ss = __shfl_sync(0xffffffffu, mystride, i);
-      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; nstride = ss; }
+      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; nstride = ss; nkeep = kp; }
     }
     bool pad = node < 0 || (node == 0 && k >= K0r);
+    int korig = 0;   // the original option index behind slot digit k (kept options only; the pinned one for a fixed node)
+    if (nfix) korig = nfk;
+    else if (!pad && ne >= 0) korig = nth_set_bit(nkeep, k);
     if (fast && nbc && node == 0) {
       // slot k = group g (backend g), position p: the p-th candidate option of node 0 on backend g
       const int g = k / G, pp = k % G;
       int found = -1, seen = 0;
       for (int kk = 0; kk < nK; kk++) {
-        if (nfix && kk != nfk) continue;
+        if (nfix ? (kk != nfk) : !((nkeep >> kk) & 1)) continue;
         const int be = (ne < 0 || (nfix && residual)) ? 0 : b.backend[no0 + kk];
         if (be == g) { if (seen == pp) found = kk; seen++; }
       }
       if (ne < 0) found = (g == 0 && pp == 0) ? 0 : -1;   // dummy node: one neutral option
       pad = found < 0;
-      k = nfix ? 0 : (found < 0 ? 0 : found);           // k = enumerated digit value (0 for a pinned node)
+      korig = found < 0 ? 0 : found;
     }
     int dl[DYPLAN_MAX_LEVELS];
 #pragma unroll
@@ -315,7 +365,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) dl[l] = INT32_MAX;
       f = -1.0f;   // a padding option can never tie or beat an incumbent: C1 * f <= 0
     } else if (ne >= 0 && !(nfix && residual)) {
-      const int o = no0 + (nfix ? nfk : k);
+      const int o = no0 + korig;
       be = b.backend[o]; dem = b.demand[o];
       const int tau = b.lat_us[o];
 #pragma unroll
@@ -333,7 +383,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
         if (l < Lp) q_nlat[s * Lp + l] = pad ? -2.0f * kBigF : -(float)dl[l < L ? l : 0];   // padded levels repeat level 0 (their threshold never admits a plan)
       q_f[s] = pad ? 0.0f : f; q_dem[s] = (float)dem; q_be[s] = be;
-      q_idxc[s] = (pad || ne < 0 || nfix) ? 0ull : (unsigned long long)k * nstride;
+      q_idxc[s] = (pad || ne < 0 || nfix) ? 0ull : (unsigned long long)korig * nstride;
       if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = (float)dem;
     }
   }

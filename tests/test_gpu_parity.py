@@ -426,3 +426,71 @@ def test_api_argument_errors(dy):
     with pytest.raises(binding.DyplanError) as e:
         ctx.dyplan_replan(dw.batch, dw.mult, dw.mult, dw.mult, 2, dw.out)   # unknown flag
     assert e.value.code == binding.ERR_ARG
+
+
+# ---- exact dominance pruning: same results, smaller enumerated space -------------
+@pytest.fixture()
+def pruning(dy):
+    binding, ctx = dy
+    ctx.dyplan_set_flags(binding.PRUNE_DOMINATED)
+    yield
+    ctx.dyplan_set_flags(0)
+
+
+@pytest.mark.parametrize("seed,L,B,caps", [(121, 1, 1, False), (122, 3, 2, True), (123, 4, 3, True), (124, 8, 2, False)])
+def test_pruned_enumeration_equals_the_full_oracle(dy, orc, pruning, seed, L, B, caps):
+    w = wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=8, B=B, M=3, L=L, caps=caps)
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    assert st["plans"] < w.n_plans_total()                      # something was pruned ...
+    check_records(orc, w, g, orc.run(w), where=f"pruned(seed={seed})")   # ... and nothing changed
+
+
+def test_pruned_configs_and_replan(dy, orc, pruning):
+    for w in (wl.make_config(0), wl.make_config(1, R=2), wl.make_config(2, R=12)):
+        g = gpu_run(dy, w)
+        st = dy[1].dyplan_last_stats()
+        c = check_records(orc, w, g, orc.run(w), where=f"pruned {w.name}")
+        assert st["plans"] <= w.n_plans_total()
+    w = wl.random_replan_workload(125, R=40, nmin=1, nmax=8, kmin=1, kmax=6, B=3, M=3, caps=True)
+    check_records(orc, w, gpu_run(dy, w), orc.run(w), where="pruned replan")
+    w.flags = wl.FLAG_RESIDUAL
+    check_records(orc, w, gpu_run(dy, w), orc.run(w), where="pruned replan residual")
+
+
+def test_pruning_with_exact_ties_keeps_the_tie_break(dy, orc, pruning):
+    # duplicated options (equal f, equal durations): only the lower index may survive, and order 7 must still hold
+    w = wl.make_config(1, R=2)
+    b = w.batch
+    b.acc[:] = np.round(b.acc * 4) / 4
+    b.vuln[:] = np.round(b.vuln * 2) / 2
+    b.lat_us[:] = (b.lat_us // 400 + 1) * 400
+    g = gpu_run(dy, w)
+    ref = orc.run(w)
+    c = check_records(orc, w, g, ref, where="pruned ties")
+    ok = ref["status"] == 0
+    assert (g["plan_idx"][ok] == ref["plan_idx"][ok]).all()
+
+
+def test_pruning_reaches_a_space_beyond_brute_force(dy, orc, pruning):
+    # 11 nodes x 16 options = 1.8e13 plans: TOO_LARGE unpruned; dominance leaves a Pareto front per node.  Optimum from
+    # the independent MILP of PIN13.
+    from test_oracle_pins import milp_best_corr
+    binding, ctx = dy
+    w = wl.random_workload(126, R=3, nmin=11, nmax=11, kmin=16, kmax=16, B=2, M=3, L=2, caps=True, tool_p=0.0, slo_q=0.4)
+    g = gpu_run(dy, w)
+    st = ctx.dyplan_last_stats()
+    assert (g["status"] != 3).all() and st["plans"] < 2**40
+    mult = np.asarray(w.mult_pm).reshape(2, 2)
+    for rec in range(6):
+        r, l = divmod(rec, 2)
+        cstar = milp_best_corr(w.batch, r, mult[l])
+        if cstar is None:
+            assert g["status"][rec] == 1
+            continue
+        assert g["status"][rec] == 0
+        c64 = float(g["corr64"][rec])
+        assert cstar * (1 - 1e-5) <= c64 <= cstar * (1 + 1e-6), (rec, c64, cstar)
+    ctx.dyplan_set_flags(0)
+    g0 = gpu_run(dy, w)
+    assert (g0["status"] == 3).all()                             # the same batch without pruning: plan space too large
