@@ -378,7 +378,7 @@ def run_linear(args, rank: int, world: int, local_rank: int):
         "e2e": {"value": world * evals * args.steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps, "api": "dyplan_compile_linear + copies"},
         "gpu_launches": st["launches"] * args.steps, "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "k_lscore (two passes)", "achieved": k_eval_s * aops / 1e12, "peak": peak,
+        "roofline": {"bound": "alu", "kernel": "k_lscore", "achieved": k_eval_s * aops / 1e12, "peak": peak,
                      "unit": "Tinst/s", "frac": k_eval_s * aops / 1e12 / peak, "traffic": None, "ops_per_eval": aops,
                      "kernel_ms": st["score_ms"]},
     }

@@ -353,25 +353,25 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   CK(cudaSetDevice(ctx->device));
   const size_t R = (size_t)in->R;
   if ((rc = ensure(ctx, ctx->lin_blob, R * kLinBlobWords * 4))) return rc;
-  if ((rc = ensure(ctx, ctx->lin_gj, R * L * 4))) return rc;
-  if ((rc = ensure(ctx, ctx->lin_gkey, R * L * 8))) return rc;
   if ((rc = ensure(ctx, ctx->lin_misc, 64))) return rc;
   LinArgs a;
   memset(&a, 0, sizeof(a));
   a.in = *in; a.out = *out; if (extra) a.extra = *extra; a.cost = cost; a.p = *params; a.L = L;
   for (int l = 0; l < L; l++) a.levels[l] = levels[l];
-  a.blob = (uint32_t*)ctx->lin_blob.p; a.gJ = (int32_t*)ctx->lin_gj.p; a.gKey = (unsigned long long*)ctx->lin_gkey.p;
+  a.blob = (uint32_t*)ctx->lin_blob.p;
   a.counter = (uint32_t*)ctx->lin_misc.p; a.plans = (unsigned long long*)((char*)ctx->lin_misc.p + 16);
   const int grid = ctx->sm_count * 8;                         // persistent-ish: work pulled from a device counter
   const uint32_t want = (uint32_t)grid * 4u * 16u;            // ~16 work items per resident warp
   uint32_t chunks = (uint32_t)((want + R - 1) / R);
   a.chunks = chunks < 1 ? 1 : (chunks > 65536u ? 65536u : chunks);
+  if ((rc = ensure(ctx, ctx->lin_gj, R * a.chunks * L * sizeof(LinRec)))) return rc;
+  a.rec = (LinRec*)ctx->lin_gj.p;
   CK(cudaMemsetAsync(ctx->lin_misc.p, 0, 64, s));
   CK(cudaEventRecord(ctx->ev0, s));
   CK(launch_linear(a, grid, s));
   CK(cudaEventRecord(ctx->ev1, s));
   ctx->have_events = true;
-  ctx->last_launches = 4;
+  ctx->last_launches = 3;
   return DYPLAN_OK;
 }
 

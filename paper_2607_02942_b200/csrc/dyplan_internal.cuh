@@ -170,6 +170,7 @@ struct LinHdr {
   unsigned long long stride[16];  // canonical stride (0 for dummies)
 };
 static_assert(sizeof(LinHdr) == kLinHdrWords * 4, "LinHdr layout");
+struct __align__(16) LinRec { float J; uint32_t pad; unsigned long long key; };   // an item's best per level
 struct LinArgs {
   dyplan_batch in;
   dyplan_bundle out;
@@ -180,8 +181,7 @@ struct LinArgs {
   float levels[DYPLAN_MAX_LEVELS];
   // scratch
   uint32_t* blob;                 // [R][kLinBlobWords]
-  int32_t* gJ;                    // [R*L] best J (order-preserving int encoding)
-  unsigned long long* gKey;       // [R*L] (T << 40 | idx) of the winner among the plans with J == best
+  LinRec* rec;                    // [R*chunks*L] item records
   uint32_t* counter;              // [2] dynamic work counters of the two passes
   uint32_t chunks;                // work items per request
   unsigned long long* plans;      // [1] total plans enumerated (stats)

@@ -3,18 +3,16 @@
 //
 //   k_lstage  one thread per request: validation, reach weights rho(n), w = rho q - lambda_f v (1-q)
 //             - lambda_c c per option, durations as exact fp32 integers
-//   k_lscore  two passes over every plan, one warp per work item (a range of outer indices of one request):
-//             pass 1 reduces max J per (request, level) (atomicMax on an order-preserving int encoding);
-//             pass 2 re-enumerates and reduces min (T, canonical index) over the plans whose J equals that maximum
-//             bit for bit (same instruction sequence), one 64-bit atomicMin of T << 40 | idx.  No thresholds, no slow path.
-//   k_lemit   one thread per (request, level): decode the winner, annotate, re-evaluate J in fp64
+//   k_lscore  every plan, one warp per work item (a range of outer indices of one request).  Each lane keeps its own
+//             incumbent per level -- best J32 and, among the plans attaining it, min (T << 40 | idx) -- in registers; the
+//             unrolled inner block only tests J >= incumbent and a group that has a hit is walked again to update.  The
+//             item's record per level = max J over the lanes, min key among the lanes attaining it (shuffles).
+//   k_lemit   one thread per (request, level): reduce the request's item records (J desc, key asc), decode the winner,
+//             annotate, re-evaluate J in fp64
 // J32 is a pure function of the plan: W is summed from the last node down, then one FFMA per term.
 #include "dyplan_common.cuh"
 
 namespace dyplan {
-
-__device__ __forceinline__ int enc_f32(float f) { int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
-__device__ __forceinline__ float dec_f32(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
 
 __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -24,7 +22,6 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
   LinHdr* h = (LinHdr*)blob;
   float2* t_wd = (float2*)(blob + kLinHdrWords);   // (w, d) per slot
-  for (int l = 0; l < L; l++) { a.gJ[r * L + l] = INT32_MIN; a.gKey[r * L + l] = ~0ull; }
 
   int st = DYPLAN_ST_OK;
   const int n0 = b.node_off[r], n1 = b.node_off[r + 1], N = n1 - n0;
@@ -111,7 +108,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
 // One warp per work item (request r, chunk c): a range of outer indices (digits of the nodes >= 3) of the request, split
 // over the lanes.  Per outer index: digits by div/mod, slack DP of the nodes >= 3 from the last node down
 // (u[i] = min(0, min_succ u[j]) - d: T = -min u); then loops over the options of nodes 2, 1, 0 with one fused step each.
-template <int PASS, int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
+template <int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
 __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
   __shared__ __align__(16) uint32_t s_blob[4][kLinBlobWords];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -125,7 +122,7 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
   long long cur_req = -1;
   for (;;) {
     uint32_t item = 0;
-    if (lane == 0) item = atomicAdd(&a.counter[PASS], 1u);
+    if (lane == 0) item = atomicAdd(&a.counter[0], 1u);
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= total) break;
     const long long r = item / a.chunks;
@@ -151,13 +148,10 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
     const unsigned long long st0 = h->stride[0], st1 = h->stride[1], st2 = h->stride[2];
     const int ob1 = h->optbase[1], ob2 = h->optbase[2];
 
-    float best[LT], tgt[LT];
+    float best[LT];                 // the lane's incumbent J per level and, among the plans attaining it, min (T << 40 | idx)
     unsigned long long kmin[LT];
 #pragma unroll
-    for (int l = 0; l < LT; l++) {
-      best[l] = -INFINITY; kmin[l] = ~0ull;
-      tgt[l] = (PASS == 1 && l < L) ? dec_f32(__ldcg(&a.gJ[r * L + l])) : __int_as_float(0x7fc00000);   // NaN never matches
-    }
+    for (int l = 0; l < LT; l++) { best[l] = -INFINITY; kmin[l] = ~0ull; }
     float u[16];
     for (unsigned long long o = ob; o < oe; o++) {
       unsigned long long t = o, idxo = 0;
@@ -202,23 +196,22 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
 #pragma unroll
             for (int l = 0; l < LT; l++) {
               const float J = fmaf(cl[l], D0, Jb);        // ... - lambda_ld L D_tau
-              if (PASS == 0) best[l] = fmaxf(best[l], J);
-              else hit |= (J == tgt[l]);
+              hit |= (J >= best[l]);
             }
           }
-          if (PASS == 1 && hit) {
-            // rare: some plan of this group attains a level's maximum -- walk the group again for (T, idx)
+          if (hit) {
+            // rare once the incumbents have risen: some plan of this group ties or beats a level's incumbent
             for (int k0 = 0; k0 < K0; k0++) {
               const float2 wd0 = t_wd[k0];
               const float m = fminf(R1, ap - wd0.y);
               const float D0 = D1 + wd0.y;
               const float Jb = fmaf(lam_l, m, W1 + wd0.x);
+              const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
 #pragma unroll
               for (int l = 0; l < LT; l++) {
-                if (l < L && fmaf(cl[l], D0, Jb) == tgt[l]) {
-                  const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
-                  kmin[l] = key < kmin[l] ? key : kmin[l];
-                }
+                const float J = fmaf(cl[l], D0, Jb);
+                if (J > best[l]) { best[l] = J; kmin[l] = key; }
+                else if (J == best[l] && key < kmin[l]) kmin[l] = key;
               }
             }
           }
@@ -228,17 +221,14 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
 #pragma unroll
     for (int l = 0; l < LT; l++) {
       if (l < L) {
-        if (PASS == 0) {
-          float v = best[l];
+        // the item's record: max J over the lanes, then min key among the lanes that attain it
+        float v = best[l];
 #pragma unroll
-          for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
-          if (lane == 0 && v > -INFINITY) atomicMax(&a.gJ[r * L + l], enc_f32(v));
-        } else {
-          unsigned long long v = kmin[l];
+        for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
+        unsigned long long kk = best[l] == v ? kmin[l] : ~0ull;
 #pragma unroll
-          for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, v, off); v = o2 < v ? o2 : v; }
-          if (lane == 0 && v != ~0ull) atomicMin(&a.gKey[r * L + l], v);
-        }
+        for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, kk, off); kk = o2 < kk ? o2 : kk; }
+        if (lane == 0) { LinRec rc; rc.J = v; rc.pad = 0; rc.key = kk; a.rec[((size_t)r * a.chunks + c) * L + l] = rc; }
       }
     }
   }
@@ -256,7 +246,13 @@ __global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
   const LinHdr* h = (const LinHdr*)(a.blob + (size_t)r * kLinBlobWords);
   if (h->status != DYPLAN_ST_OK) return;   // sentinels were written by k_lstage
   const dyplan_bundle& o = a.out;
-  const unsigned long long key = a.gKey[rec];
+  float bestJ = -INFINITY;
+  unsigned long long key = ~0ull;
+  for (uint32_t c = 0; c < a.chunks; c++) {
+    const LinRec rc = a.rec[((size_t)r * a.chunks + c) * L + l];
+    if (rc.key == ~0ull) continue;                         // an item whose range was empty
+    if (rc.J > bestJ || (rc.J == bestJ && rc.key < key)) { bestJ = rc.J; key = rc.key; }
+  }
   unsigned long long idx = key & ((1ull << 40) - 1);
   const int n0 = b.node_off[r], N = h->n_orig;
   uint32_t reach[16], succ[16];
@@ -296,7 +292,7 @@ __global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
   for (int m = 1; m < M; m++) if (Dm[m] > Dm[dmod]) dmod = m;
   const double J = __dsub_rn(__dsub_rn(W, __dmul_rn((double)a.p.lambda_l, (double)T)),
                              __dmul_rn(__dmul_rn((double)a.p.lambda_ld, (double)a.levels[l]), (double)Dt));
-  o.corr[rec] = dec_f32(a.gJ[rec]);
+  o.corr[rec] = bestJ;
   if (o.corr64) o.corr64[rec] = J;
   o.lat[rec] = (int)T;
   for (int bb = 0; bb < B; bb++) o.dem[rec * B + bb] = D[bb];
@@ -310,9 +306,9 @@ cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s) {
   if (a.in.R == 0) return cudaSuccess;
   k_lstage<<<(unsigned)((a.in.R + 127) / 128), 128, 0, s>>>(a);
   switch (level_class(a.L)) {
-#define DYPLAN_LCASE(LT_) case LT_: k_lscore<0, LT_><<<grid, 128, 0, s>>>(a); k_lscore<1, LT_><<<grid, 128, 0, s>>>(a); break;
+#define DYPLAN_LCASE(LT_) case LT_: k_lscore<LT_><<<grid, 128, 0, s>>>(a); break;
     DYPLAN_LCASE(1) DYPLAN_LCASE(2) DYPLAN_LCASE(3) DYPLAN_LCASE(4) DYPLAN_LCASE(6)
-    default: k_lscore<0, 8><<<grid, 128, 0, s>>>(a); k_lscore<1, 8><<<grid, 128, 0, s>>>(a); break;
+    default: k_lscore<8><<<grid, 128, 0, s>>>(a); break;
 #undef DYPLAN_LCASE
   }
   const long long nrec = (long long)a.in.R * a.L;
