@@ -217,7 +217,8 @@ DYPLAN_API int dyplan_bind(dyplan_ctx* ctx, const dyplan_profiles* prof, int32_t
  * levels weight a demand penalty) and D_tau = sum_n tau(n, k_n).  Ties: T ascending, then canonical
  * index ascending.  Reads in->lat_us (tau), in->acc (q), in->vuln (v), in->demand / backend / model (annotations);
  * in->slo_us and in->cap are ignored (the paper's latency charge is soft).  cost: [KK] DEVICE pointer, c >= 0.
- * params and levels are HOST pointers (levels[L], ascending from 0 in the paper; any finite values >= 0 accepted).
+ * params and levels are HOST pointers (levels[L], ascending from 0 in the paper; any values in [0, 1e6] accepted, as for
+ * the weights).
  * out: one record per (request, level); corr = J as the scorer computed it (fp32), corr64 = J re-evaluated in fp64,
  * lat = T, dem / dom_model as in dyplan_compile.  extra (optional, DEVICE arrays): dtau [R*L] = D_tau of the chosen
  * plan, quality [R*L] = prod_n (1 - v_n (1 - q)) of the chosen plan (the variant's quality estimate dyplan_switch uses).

@@ -347,9 +347,9 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   if (!params || !levels || (in->KK > 0 && !cost)) return DYPLAN_ERR_NULL;
   if ((rc = check_bundle(out))) return rc;
   const float pv[6] = {params->lambda_f, params->lambda_c, params->lambda_l, params->lambda_ld, params->beta, params->effort};
-  for (float v : pv) if (!(v >= 0.0f) || v > 1e30f) return DYPLAN_ERR_ARG;
+  for (float v : pv) if (!(v >= 0.0f) || v > 1e6f) return DYPLAN_ERR_ARG;   // (padding options score -1e30)
   if (params->effort > 1.0f) return DYPLAN_ERR_ARG;
-  for (int l = 0; l < L; l++) if (!(levels[l] >= 0.0f) || levels[l] > 1e30f) return DYPLAN_ERR_ARG;
+  for (int l = 0; l < L; l++) if (!(levels[l] >= 0.0f) || levels[l] > 1e6f) return DYPLAN_ERR_ARG;
   CK(cudaSetDevice(ctx->device));
   const size_t R = (size_t)in->R;
   if ((rc = ensure(ctx, ctx->lin_blob, R * kLinBlobWords * 4))) return rc;
@@ -361,11 +361,13 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   a.blob = (uint32_t*)ctx->lin_blob.p;
   a.counter = (uint32_t*)ctx->lin_misc.p; a.plans = (unsigned long long*)((char*)ctx->lin_misc.p + 16);
   const int grid = ctx->sm_count * 8;                         // persistent-ish: work pulled from a device counter
-  const uint32_t want = (uint32_t)grid * 4u * 16u;            // ~16 work items per resident warp
+  const uint32_t want = (uint32_t)grid * 4u * 6u;             // ~6 work items per launched warp
   uint32_t chunks = (uint32_t)((want + R - 1) / R);
   a.chunks = chunks < 1 ? 1 : (chunks > 65536u ? 65536u : chunks);
   if ((rc = ensure(ctx, ctx->lin_gj, R * a.chunks * L * sizeof(LinRec)))) return rc;
   a.rec = (LinRec*)ctx->lin_gj.p;
+  if ((rc = ensure(ctx, ctx->lin_gkey, R * L * 4))) return rc;
+  a.gJ = (int32_t*)ctx->lin_gkey.p;
   CK(cudaMemsetAsync(ctx->lin_misc.p, 0, 64, s));
   CK(cudaEventRecord(ctx->ev0, s));
   CK(launch_linear(a, grid, s));

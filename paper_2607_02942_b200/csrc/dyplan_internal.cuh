@@ -182,6 +182,7 @@ struct LinArgs {
   // scratch
   uint32_t* blob;                 // [R][kLinBlobWords]
   LinRec* rec;                    // [R*chunks*L] item records
+  int32_t* gJ;                    // [R*L] best J published so far (order-preserving int encoding)
   uint32_t* counter;              // [2] dynamic work counters of the two passes
   uint32_t chunks;                // work items per request
   unsigned long long* plans;      // [1] total plans enumerated (stats)

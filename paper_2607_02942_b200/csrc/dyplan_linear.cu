@@ -14,6 +14,10 @@
 
 namespace dyplan {
 
+// order-preserving int encoding of a float (for atomicMax on the best J published per (request, level))
+__device__ __forceinline__ int enc_f32(float f) { int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
+__device__ __forceinline__ float dec_f32(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
+
 __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const dyplan_batch& b = a.in;
@@ -22,6 +26,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
   LinHdr* h = (LinHdr*)blob;
   float2* t_wd = (float2*)(blob + kLinHdrWords);   // (w, d) per slot
+  for (int l = 0; l < L; l++) a.gJ[r * L + l] = enc_f32(-INFINITY);
 
   int st = DYPLAN_ST_OK;
   const int n0 = b.node_off[r], n1 = b.node_off[r + 1], N = n1 - n0;
@@ -108,16 +113,144 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
 // One warp per work item (request r, chunk c): a range of outer indices (digits of the nodes >= 3) of the request, split
 // over the lanes.  Per outer index: digits by div/mod, slack DP of the nodes >= 3 from the last node down
 // (u[i] = min(0, min_succ u[j]) - d: T = -min u); then loops over the options of nodes 2, 1, 0 with one fused step each.
+// One work item (request r, chunk c) for one lane of the warp; LT = padded level count, K0P = node 0's radix class.
+template <int LT, int K0P>
+__device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArgs& a, long long r, uint32_t c, const float* __restrict__ clp,
+                                   float lam_l) {
+  const int lane = threadIdx.x & 31;
+  const int L = a.L;
+  const LinHdr* h = (const LinHdr*)sb;
+  const int K0 = h->K[0];
+  float cl[LT];
+#pragma unroll
+  for (int l = 0; l < LT; l++) cl[l] = clp[l];
+  const float2* t_wd = (const float2*)(sb + kLinHdrWords);   // (w, d) per slot
+  const unsigned long long outer = h->outer_total;            // prod_{i>=3} K_i
+  const unsigned long long per = (((outer + a.chunks - 1) / a.chunks + 31) / 32) * 32;   // a whole number of outer indices per lane
+  const unsigned long long cb = min((unsigned long long)c * per, outer), ce = min(cb + per, outer);
+  const unsigned long long lper = (ce - cb + 31) / 32;
+  const unsigned long long ob = min(cb + lane * lper, ce), oe = min(ob + lper, ce);
+  const int Np = h->n_int, K1 = h->K[1], K2 = h->K[2];
+  const uint32_t succ0 = h->succ[0], succ1 = h->succ[1], succ2 = h->succ[2];
+  const bool c01 = (succ0 >> 1) & 1, c02 = (succ0 >> 2) & 1, c12 = (succ1 >> 2) & 1;
+  const unsigned long long st0 = h->stride[0], st1 = h->stride[1], st2 = h->stride[2];
+  const int ob1 = h->optbase[1], ob2 = h->optbase[2];
+
+  float w0[K0P], d0[K0P];         // node 0's tables in registers (padding options: w = -1e30, never an incumbent)
+#pragma unroll
+  for (int k = 0; k < K0P; k++) { const float2 wd = t_wd[k < K0 ? k : 0]; w0[k] = k < K0 ? wd.x : -1e30f; d0[k] = k < K0 ? wd.y : 0.0f; }
+  float best[LT];                 // the lane's incumbent J per level and, among the plans attaining it, min (T << 40 | idx)
+  unsigned long long kmin[LT];
+#pragma unroll
+  // the incumbent starts from the best J any finished item of this request has published: a J some plan attains, so
+  // plans below it can never win and plans that tie it still pass the test (the key decides); kmin stays ~0 until
+  // one of THIS lane's plans ties or beats it
+  for (int l = 0; l < LT; l++) { best[l] = l < L ? dec_f32(__ldcg(&a.gJ[r * L + l])) : INFINITY; kmin[l] = ~0ull; }
+
+  float u[16];
+  for (unsigned long long step = 0; step < lper; step++) {   // the same trip count on every lane: the loop shuffles
+    // share the climb: every lane's incumbent rises to the best J any lane of the warp has reached (a lane whose
+    // incumbent is raised by another lane's plan no longer holds a plan attaining it: its key is cleared)
+#pragma unroll
+    for (int l = 0; l < LT; l++) {
+      float v = best[l];
+#pragma unroll
+      for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
+      if (v > best[l]) { best[l] = v; kmin[l] = ~0ull; }
+    }
+    const unsigned long long o = ob + step;
+    if (o >= oe) continue;
+    unsigned long long t = o, idxo = 0;
+    int dig[16];
+    for (int i = 3; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
+    float Wp = 0.0f, Dp = 0.0f, Rm = 0.0f;
+    for (int i = Np - 1; i >= 3; --i) {
+      const float2 wd = t_wd[h->optbase[i] + dig[i]];
+      float m = 0.0f;
+      for (uint32_t dm = h->succ[i]; dm; dm &= dm - 1) m = fminf(m, u[__ffs(dm) - 1]);
+      u[i] = m - wd.y;
+      Rm = fminf(Rm, u[i]);
+      Wp += wd.x;
+      Dp += wd.y;
+    }
+    float u2in = 0.0f, u1in3 = 0.0f, a0in3 = 0.0f;
+    for (uint32_t dm = succ2; dm; dm &= dm - 1) u2in = fminf(u2in, u[__ffs(dm) - 1]);
+    for (uint32_t dm = succ1 & ~7u; dm; dm &= dm - 1) u1in3 = fminf(u1in3, u[__ffs(dm) - 1]);
+    for (uint32_t dm = succ0 & ~7u; dm; dm &= dm - 1) a0in3 = fminf(a0in3, u[__ffs(dm) - 1]);
+    for (int k2 = 0; k2 < K2; k2++) {
+      const float2 wd2 = t_wd[ob2 + k2];
+      const float u2 = u2in - wd2.y;
+      const float R2 = fminf(Rm, u2);
+      const float W2 = Wp + wd2.x, D2 = Dp + wd2.y;
+      const float u1in = c12 ? fminf(u1in3, u2) : u1in3;
+      const float a0in = c02 ? fminf(a0in3, u2) : a0in3;
+      const unsigned long long idx2 = idxo + (unsigned long long)k2 * st2;
+      for (int k1 = 0; k1 < K1; k1++) {
+        const float2 wd1 = t_wd[ob1 + k1];
+        const float u1 = u1in - wd1.y;
+        const float R1 = fminf(R2, u1);
+        const float W1 = W2 + wd1.x, D1 = D2 + wd1.y;
+        const float ap = c01 ? fminf(a0in, u1) : a0in;
+        const unsigned long long idx1 = idx2 + (unsigned long long)k1 * st1;
+        // screen: h > = 0 iff some (plan, level) of the group ties or beats the lane's incumbent (J - best has an exact sign)
+        float h = -1.0f;
+#pragma unroll
+        for (int k0 = 0; k0 < K0P; k0++) {
+          const float m = fminf(R1, ap - d0[k0]);        // least slack = -T
+          const float D0 = D1 + d0[k0];
+          const float Jb = fmaf(lam_l, m, W1 + w0[k0]);  // W - lambda_l T
+          float dj[LT];
+#pragma unroll
+          for (int l = 0; l < LT; l++) dj[l] = fmaf(cl[l], D0, Jb) - best[l];   // J - incumbent
+#pragma unroll
+          for (int l = 0; l + 1 < LT; l += 2) h = fmaxf(h, fmaxf(dj[l], dj[l + 1]));
+          if (LT & 1) h = fmaxf(h, dj[LT - 1]);
+        }
+        if (__builtin_expect(h >= 0.0f, 0)) {
+          // rare once the incumbents have risen: walk the group again and update
+#pragma unroll 1
+          for (int k0 = 0; k0 < K0; k0++) {
+            const float2 wd0 = t_wd[k0];
+            const float m = fminf(R1, ap - wd0.y);
+            const float D0 = D1 + wd0.y;
+            const float Jb = fmaf(lam_l, m, W1 + wd0.x);
+            const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
+#pragma unroll
+            for (int l = 0; l < LT; l++) {
+              const float J = fmaf(cl[l], D0, Jb);
+              if (J > best[l]) { best[l] = J; kmin[l] = key; }
+              else if (J == best[l] && key < kmin[l]) kmin[l] = key;
+            }
+          }
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int l = 0; l < LT; l++) {
+    if (l < L) {
+      // the item's record: max J over the lanes, then min key among the lanes that attain it
+      float v = best[l];
+#pragma unroll
+      for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
+      unsigned long long kk = best[l] == v ? kmin[l] : ~0ull;
+#pragma unroll
+      for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, kk, off); kk = o2 < kk ? o2 : kk; }
+      if (lane == 0) { LinRec rc; rc.J = v; rc.pad = 0; rc.key = kk; a.rec[((size_t)r * a.chunks + c) * L + l] = rc; }
+    }
+  }
+}
+
 template <int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
 __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
   __shared__ __align__(16) uint32_t s_blob[4][kLinBlobWords];
+  __shared__ float s_cl[8];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   uint32_t* sb = s_blob[wid];
   const int L = a.L;
   const uint32_t total = (uint32_t)a.in.R * a.chunks;
-  float cl[LT];
-#pragma unroll
-  for (int l = 0; l < LT; l++) cl[l] = l < L ? -(a.p.lambda_ld * a.levels[l]) : 0.0f;
+  if (threadIdx.x < 8) s_cl[threadIdx.x] = (int)threadIdx.x < L ? -(a.p.lambda_ld * a.levels[threadIdx.x]) : 0.0f;
+  __syncthreads();
   const float lam_l = a.p.lambda_l;
   long long cur_req = -1;
   for (;;) {
@@ -136,101 +269,13 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
     }
     const LinHdr* h = (const LinHdr*)sb;
     if (h->status != DYPLAN_ST_OK) continue;
-    const float2* t_wd = (const float2*)(sb + kLinHdrWords);   // (w, d) per slot
-    const unsigned long long outer = h->outer_total;            // prod_{i>=3} K_i
-    const unsigned long long per = (outer + a.chunks - 1) / a.chunks;
-    const unsigned long long cb = min((unsigned long long)c * per, outer), ce = min(cb + per, outer);
-    const unsigned long long lper = (ce - cb + 31) / 32;
-    const unsigned long long ob = min(cb + lane * lper, ce), oe = min(ob + lper, ce);
-    const int Np = h->n_int, K0 = h->K[0], K1 = h->K[1], K2 = h->K[2];
-    const uint32_t succ0 = h->succ[0], succ1 = h->succ[1], succ2 = h->succ[2];
-    const bool c01 = (succ0 >> 1) & 1, c02 = (succ0 >> 2) & 1, c12 = (succ1 >> 2) & 1;
-    const unsigned long long st0 = h->stride[0], st1 = h->stride[1], st2 = h->stride[2];
-    const int ob1 = h->optbase[1], ob2 = h->optbase[2];
-
-    float best[LT];                 // the lane's incumbent J per level and, among the plans attaining it, min (T << 40 | idx)
-    unsigned long long kmin[LT];
-#pragma unroll
-    for (int l = 0; l < LT; l++) { best[l] = -INFINITY; kmin[l] = ~0ull; }
-    float u[16];
-    for (unsigned long long o = ob; o < oe; o++) {
-      unsigned long long t = o, idxo = 0;
-      int dig[16];
-      for (int i = 3; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
-      float Wp = 0.0f, Dp = 0.0f, Rm = 0.0f;
-      for (int i = Np - 1; i >= 3; --i) {
-        const float2 wd = t_wd[h->optbase[i] + dig[i]];
-        float m = 0.0f;
-        for (uint32_t dm = h->succ[i]; dm; dm &= dm - 1) m = fminf(m, u[__ffs(dm) - 1]);
-        u[i] = m - wd.y;
-        Rm = fminf(Rm, u[i]);
-        Wp += wd.x;
-        Dp += wd.y;
-      }
-      float u2in = 0.0f, u1in3 = 0.0f, a0in3 = 0.0f;
-      for (uint32_t dm = succ2; dm; dm &= dm - 1) u2in = fminf(u2in, u[__ffs(dm) - 1]);
-      for (uint32_t dm = succ1 & ~7u; dm; dm &= dm - 1) u1in3 = fminf(u1in3, u[__ffs(dm) - 1]);
-      for (uint32_t dm = succ0 & ~7u; dm; dm &= dm - 1) a0in3 = fminf(a0in3, u[__ffs(dm) - 1]);
-      for (int k2 = 0; k2 < K2; k2++) {
-        const float2 wd2 = t_wd[ob2 + k2];
-        const float u2 = u2in - wd2.y;
-        const float R2 = fminf(Rm, u2);
-        const float W2 = Wp + wd2.x, D2 = Dp + wd2.y;
-        const float u1in = c12 ? fminf(u1in3, u2) : u1in3;
-        const float a0in = c02 ? fminf(a0in3, u2) : a0in3;
-        const unsigned long long idx2 = idxo + (unsigned long long)k2 * st2;
-        for (int k1 = 0; k1 < K1; k1++) {
-          const float2 wd1 = t_wd[ob1 + k1];
-          const float u1 = u1in - wd1.y;
-          const float R1 = fminf(R2, u1);
-          const float W1 = W2 + wd1.x, D1 = D2 + wd1.y;
-          const float ap = c01 ? fminf(a0in, u1) : a0in;
-          const unsigned long long idx1 = idx2 + (unsigned long long)k1 * st1;
-          bool hit = false;
-#pragma unroll 4
-          for (int k0 = 0; k0 < K0; k0++) {
-            const float2 wd0 = t_wd[k0];
-            const float m = fminf(R1, ap - wd0.y);        // least slack = -T
-            const float D0 = D1 + wd0.y;
-            const float Jb = fmaf(lam_l, m, W1 + wd0.x);  // W - lambda_l T
-#pragma unroll
-            for (int l = 0; l < LT; l++) {
-              const float J = fmaf(cl[l], D0, Jb);        // ... - lambda_ld L D_tau
-              hit |= (J >= best[l]);
-            }
-          }
-          if (hit) {
-            // rare once the incumbents have risen: some plan of this group ties or beats a level's incumbent
-            for (int k0 = 0; k0 < K0; k0++) {
-              const float2 wd0 = t_wd[k0];
-              const float m = fminf(R1, ap - wd0.y);
-              const float D0 = D1 + wd0.y;
-              const float Jb = fmaf(lam_l, m, W1 + wd0.x);
-              const unsigned long long key = ((unsigned long long)(-m) << 40) | (idx1 + (unsigned long long)k0 * st0);
-#pragma unroll
-              for (int l = 0; l < LT; l++) {
-                const float J = fmaf(cl[l], D0, Jb);
-                if (J > best[l]) { best[l] = J; kmin[l] = key; }
-                else if (J == best[l] && key < kmin[l]) kmin[l] = key;
-              }
-            }
-          }
-        }
-      }
-    }
-#pragma unroll
-    for (int l = 0; l < LT; l++) {
-      if (l < L) {
-        // the item's record: max J over the lanes, then min key among the lanes that attain it
-        float v = best[l];
-#pragma unroll
-        for (int off = 16; off; off >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, off));
-        unsigned long long kk = best[l] == v ? kmin[l] : ~0ull;
-#pragma unroll
-        for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, kk, off); kk = o2 < kk ? o2 : kk; }
-        if (lane == 0) { LinRec rc; rc.J = v; rc.pad = 0; rc.key = kk; a.rec[((size_t)r * a.chunks + c) * L + l] = rc; }
-      }
-    }
+    const int k0 = h->K[0];
+    if (k0 <= 2) litem<LT, 2>(sb, a, r, c, s_cl, lam_l);
+    else if (k0 <= 4) litem<LT, 4>(sb, a, r, c, s_cl, lam_l);
+    else if (k0 <= 6) litem<LT, 6>(sb, a, r, c, s_cl, lam_l);
+    else if (k0 <= 8) litem<LT, 8>(sb, a, r, c, s_cl, lam_l);
+    else if (k0 <= 12) litem<LT, 12>(sb, a, r, c, s_cl, lam_l);
+    else litem<LT, 16>(sb, a, r, c, s_cl, lam_l);
   }
 }
 
