@@ -30,6 +30,10 @@ sys.path.insert(0, ROOT)
 METRIC = "plan_level_evaluations_per_s"
 UNIT = "Geval/s"
 SM_LANES = 128            # FP32/INT32 lanes per SM = 4 SMSPs x 32 (one warp instruction per clock per SMSP)
+# dram__bytes_read.sum + dram__bytes_write.sum of the scoring kernel, per launch, from the `ncu --set full` captures of
+# profiles/r1e_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
+# (cfg4's is local-memory write-back).  None for a workload that was not captured (cfg0, down-scaled runs).
+NCU_DRAM_BYTES = {1: 25.74e6, 2: 49.58e6, 3: 96.25e6, 4: 393.49e6}
 
 
 def alg_ops_per_eval(w) -> float:
@@ -272,7 +276,8 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": "k_fscore" if st.get("fast_requests", 0) else "k_score", "achieved": achieved, "peak": peak, "unit": "Tinst/s",
-                     "frac": achieved / peak, "traffic": None,
+                     "frac": achieved / peak,
+                     "traffic": NCU_DRAM_BYTES.get(args.config) if args.requests is None else None,
                      "ops_per_eval": aops, "kernel_ms": k_ms / args.steps,
                      "peak_how": f"{sm_count} SMs x 128 lanes x {sm_max:.0f} MHz (B300_MICROARCH.md: 1 warp-inst/clk/SMSP); DESIGN.md section 8"},
     }
