@@ -480,16 +480,20 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   const size_t blob_stride = blob_stride_words(a.L);
   const long long chunk = (R + 1023) / 1024;
   const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
-  unsigned long long so = 0, sf = 0, sp = 0;
+  unsigned long long so = 0, sf = 0, sp = 0, mxf = 0;
   uint32_t nf = 0;
+  __shared__ unsigned long long s_mxf;
+  if (tid == 0) s_mxf = 0;
+  __syncthreads();
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     if (h->status == DYPLAN_ST_OK) {
-      if (h->klass == kClassFast) { sf += h->outer_total; nf++; } else so += h->outer_total;
+      if (h->klass == kClassFast) { sf += h->outer_total; nf++; mxf = h->outer_total > mxf ? h->outer_total : mxf; } else so += h->outer_total;
       sp += h->outer_total * (unsigned long long)(h->K0 * h->K1);
     }
   }
   s_sum[tid] = so; s_sumf[tid] = sf; s_plans[tid] = sp; s_nf[tid] = nf;
+  if (mxf) atomicMax(&s_mxf, mxf);
   __syncthreads();
   for (int off = 512; off; off >>= 1) {
     if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_sumf[tid] += s_sumf[tid + off]; s_plans[tid] += s_plans[tid + off]; s_nf[tid] += s_nf[tid + off]; }
@@ -506,13 +510,16 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   pio = ((pio + kBlock - 1) / kBlock) * kBlock;
   if (pio < (unsigned long long)kBlock) pio = kBlock;
   // fast: outer indices per item, a multiple of the warp size; target_items_f items when there is enough work
-  const unsigned long long tgt = a.target_items_f ? a.target_items_f : 1;
+  // requests of very different sizes (replan queries with 4 to 7 free nodes) balance better with more, smaller items
+  const bool uneven = n_fast > 0 && s_mxf > 2 * (total_f / n_fast);
+  const unsigned long long tgt0 = a.target_items_f ? a.target_items_f : 1;
+  const unsigned long long tgt = uneven ? tgt0 + tgt0 / 2 : tgt0;
   unsigned long long pif = (total_f + tgt - 1) / tgt;
   need = (total_f + budget - 1) / budget;
   if (need > pif) pif = need;
   // small calls: an item should carry at least 8 outer indices per lane (its fixed cost is a few thousand instructions)
   // unless that would leave resident warps without work (target_items_f = 24 items per resident warp)
-  const unsigned long long warps = tgt / 24 ? tgt / 24 : 1;
+  const unsigned long long warps = a.target_items_f / 16 ? a.target_items_f / 16 : 1;
   unsigned long long floor_f = (total_f + warps - 1) / warps;
   floor_f = floor_f > 256 ? 256 : floor_f;
   if (floor_f > pif) pif = floor_f;
