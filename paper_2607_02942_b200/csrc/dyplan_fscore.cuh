@@ -363,6 +363,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
   const uint32_t total_items = a.st->total_items_f;
   const uint32_t rec_base = a.st->total_items;          // partial records of the wide class come first
   const unsigned long long pif = a.st->per_item_outer_f;
+  const bool small_call = a.st->small_call_f != 0;
   if (lane == 0) mbar_init(&ws->bar, 1);
   __syncwarp();
   uint32_t phase = 0;
@@ -398,7 +399,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (lane < 8) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; ws->best[lane] = e; }
     __syncwarp();
     const uint32_t first_item = __ldg(&a.item_off_f[r]);
-    const unsigned long long pir = fast_item_outer(pif, h->Kp[2]);
+    const unsigned long long pir = fast_item_outer(pif, h->Kp[2], small_call);
     const unsigned long long ob = (unsigned long long)(item - first_item) * pir;
     const unsigned long long oe = min(ob + pir, (unsigned long long)h->outer_total);
     const unsigned long long len = oe - ob;
@@ -406,7 +407,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     // the same k2 and the heavy steps coincide); every lane runs `per` steps, the ones past its range score nothing
     const unsigned long long K2u = (unsigned long long)h->Kp[2];
     const unsigned long long per0 = (len + 31) / 32;
-    const unsigned long long per = per0 < 4 * K2u ? per0 : ((per0 + K2u - 1) / K2u) * K2u;
+    const unsigned long long per = per0 < 2 * K2u ? per0 : ((per0 + K2u - 1) / K2u) * K2u;   // (short ranges: all lanes busy beats lanes in phase)
     const unsigned long long tb = min(ob + (unsigned long long)lane * per, oe);
     const unsigned long long te = min(tb + per, oe);
     {

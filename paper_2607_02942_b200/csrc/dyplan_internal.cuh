@@ -25,9 +25,9 @@ constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp work
 constexpr float kBigF = 16777216.0f; // 2^24
 // fast class: outer indices per work item of a request whose node 2 has K2 options -- the call-wide figure rounded up
 // so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)
-__host__ __device__ inline unsigned long long fast_item_outer(unsigned long long pif, int K2) {
+__host__ __device__ inline unsigned long long fast_item_outer(unsigned long long pif, int K2, bool small_call) {
   const unsigned long long q = 32ull * (unsigned long long)(K2 < 1 ? 1 : K2);
-  if (pif < 4 * q) return ((pif + 31) / 32) * 32;   // small calls: favour more items over aligned lanes
+  if (small_call) return ((pif + 31) / 32) * 32;   // too little work to fill the GPU: favour more items over aligned lanes
   return ((pif + q - 1) / q) * q;
 }
 __host__ __device__ inline int level_class(int L) { return L <= 4 ? L : (L <= 6 ? 6 : 8); }
@@ -86,7 +86,7 @@ struct CallState {
   uint32_t total_items_f;           // fast class
   uint32_t next_item_f;
   uint32_t fast_requests;           // requests staged for the fp32 scorer
-  uint32_t pad;
+  uint32_t small_call_f;            // fast class: fewer than ~1K outer indices per resident warp (items are not lane-aligned)
 };
 
 struct CallArgs {                   // passed by value to the kernels

@@ -525,11 +525,12 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   if (floor_f > pif) pif = floor_f;
   pif = ((pif + 31) / 32) * 32;
   if (pif < 32) pif = 32;
+  const bool small_f = total_f / warps < 1024;   // not enough outer indices for one lane-aligned item per resident warp
   uint32_t cw = 0, cf = 0;
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     if (h->status != DYPLAN_ST_OK) continue;
-    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2]); cf += (uint32_t)((h->outer_total + q - 1) / q); }
+    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2], small_f); cf += (uint32_t)((h->outer_total + q - 1) / q); }
     else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
   uint32_t runw = block_exclusive_scan_1024(s_cnt, tid, cw);
@@ -542,7 +543,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     a.item_off[r] = runw;
     a.item_off_f[r] = runf;
     if (h->status != DYPLAN_ST_OK) continue;
-    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2]); runf += (uint32_t)((h->outer_total + q - 1) / q); }
+    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(pif, h->Kp[2], small_f); runf += (uint32_t)((h->outer_total + q - 1) / q); }
     else runw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
   if (tid == 1023) {
@@ -552,7 +553,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
     st->slow_steps = 0;
     st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
-    st->fast_requests = n_fast; st->pad = 0;
+    st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u;
   }
 }
 
