@@ -37,7 +37,7 @@ NCU_DRAM_BYTES = {1: 25.74e6, 2: 49.58e6, 3: 96.25e6, 4: 393.49e6}
 
 
 def alg_ops_per_eval(w) -> float:
-    """Algorithmic thread-instructions per (plan, level) evaluation, SURVEY.md 8(d) D.4 / DESIGN.md section 8:
+    """Algorithmic thread-instructions per (plan, level) evaluation, SURVEY.md 8(d) D.4 / DESIGN.md section 9:
     per (plan, level) one add(-max), one SLO compare, one best compare; per plan one multiply, one demand add and
     B cap compares (only when caps exist); outer-digit repairs are amortised by 1/K and not counted."""
     nb = w.batch.B if w.batch.cap is not None else 0
@@ -279,7 +279,7 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
                      "frac": achieved / peak,
                      "traffic": NCU_DRAM_BYTES.get(args.config) if args.requests is None else None,
                      "ops_per_eval": aops, "kernel_ms": k_ms / args.steps,
-                     "peak_how": f"{sm_count} SMs x 128 lanes x {sm_max:.0f} MHz (B300_MICROARCH.md: 1 warp-inst/clk/SMSP); DESIGN.md section 8"},
+                     "peak_how": f"{sm_count} SMs x 128 lanes x {sm_max:.0f} MHz (B300_MICROARCH.md: 1 warp-inst/clk/SMSP); DESIGN.md section 9"},
     }
     if world == 1 and not args.no_cpu_baseline:
         sample = oracle_sample(w, args.cpu_requests)

@@ -4,7 +4,7 @@
 // Same walk as k_score (dyplan_score.cuh), but
 //   * the slack DP of Eq.(3) runs on exact fp32 integers (k_stage admits a request only when every slack, latency
 //     and demand sum stays below 2^22), because on sm_100a FADD/FMUL/FFMA issue at 1 warp-instruction/clk/SMSP
-//     while IADD3/LOP3/VIADDMNMX/IMAD issue at 0.5 (measured, profiles/r1c_m0_pipe_rates.md);
+//     while IADD3/LOP3/VIADDMNMX/IMAD issue at 0.5 (measured on this B200);
 //   * the work item belongs to one WARP, not one block: no block barrier anywhere in the loop;
 //   * per (plan, level) the screen is two FMA-pipe instructions and half an ALU-pipe instruction:
 //         x = sat(ap1_l - d0[k0][l])          FADD.SAT   1 iff node 0 (hence every node) meets the SLO at level l
@@ -12,7 +12,7 @@
 //         zmax = max3(zmax, z, z')            FMNMX3     one per two evaluations
 //     with P = C1 * f0[k0] (one FMUL per plan; with caps P is also multiplied by x_cap = sat(slackD_g + 1 - dem0[k0]),
 //     node 0's options being laid out in one slot group per backend).  A group whose zmax > 0 is re-walked by the
-//     exact slow path (order 7 with T and the canonical index), which updates the lane's incumbent.
+//     exact, warp-cooperative slow path (order 7 with T and the canonical index), which updates the warp's incumbent.
 #pragma once
 #include "dyplan_common.cuh"
 

@@ -1,5 +1,5 @@
 // dyplan_internal.cuh -- structures shared by the kernels of libdyplan (product side only; the oracle
-// shares nothing with this directory).  See DESIGN.md sections 4-6 for the layout and the kernels.
+// shares nothing with this directory).  See DESIGN.md sections 6-7 for the layout and the kernels.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -32,7 +32,7 @@ __host__ __device__ inline unsigned long long fast_item_outer(unsigned long long
 }
 __host__ __device__ inline int level_class(int L) { return L <= 4 ? L : (L <= 6 ? 6 : 8); }
 
-// Per-request staged problem in "internal" node order (DESIGN.md 5.1).  Internal node 0 is the innermost
+// Per-request staged problem in "internal" node order (DESIGN.md 6.1).  Internal node 0 is the innermost
 // enumeration digit, node 1 the middle digit, nodes >= 2 the outer digits.  deps(i) only holds nodes j > i, so
 // the slack recurrence  u[i] = min(SLO, min_{j in deps(i)} u[j]) - d[i][k_i]  can be evaluated from the
 // outermost node inwards; the longest path is  T = SLO - min_i u[i]  (Eq.(3), in slack form).

@@ -1,5 +1,5 @@
 // dyplan_score.cuh -- K_score: enumerate + score + arg-best, one template per (L, NB).
-// Included by dyplan_score_l<L>.cu with DYPLAN_SCORE_L defined.  DESIGN.md section 6 explains the kernel.
+// Included by dyplan_score_l<L>.cu with DYPLAN_SCORE_L defined.  DESIGN.md 7.2 explains the kernel (the int32 scorer of the wide class).
 //
 // Per work item (a range of outer indices of one request) every thread walks its outer digits in odometer
 // order, keeps the slack DP of the outer nodes in local arrays, runs the middle digit (internal node 1) as a

@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     return;
   }
 
-  // ---- internal order (DESIGN.md 5.1) ----
+  // ---- internal order (DESIGN.md 6.1) ----
   const int Kfirst = N ? (((fmask >> 0) & 1) ? 1 : K[0]) : 1;
   int Klast = 1;
 #pragma unroll
