@@ -18,18 +18,24 @@
 
 namespace dyplan {
 
+#ifndef CTX_SHARED_MIN_L
+#define CTX_SHARED_MIN_L 4
+#endif
 template <int L>
 struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
   Best best[8];                    // the warp's incumbent per level (written by the cooperative slow path only)
   int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
   float scr[40];                   // slow path: the flagged lane's group state, broadcast through shared memory
-  float ctx[(L >= 6 ? 4 * L * 32 : 32)];   // (L >= 6 only) [4 l + v][lane]: node-2 context of every lane (X2, Rm3, U1r, A0r per level), written
+  float4 ctx[(L >= CTX_SHARED_MIN_L ? L * 32 : 1)];   // (L >= CTX_SHARED_MIN_L) [l][lane] = {X2, Rm3, U1r, A0r}: node-2 context of every lane, written
                                    // by the heavy step and read by each light step (kept out of the register file)
   unsigned long long bar;          // mbarrier of the TMA copy
   unsigned long long pad;
 };
 
+#ifndef CTX_SHARED_MIN_L
+#define CTX_SHARED_MIN_L 4
+#endif
 // scratch layout of the cooperative slow path
 constexpr int kScrC1 = 0, kScrS1 = 1, kScrAp1 = 9, kScrU1 = 17, kScrR2 = 25, kScrIdx = 34;
 
@@ -101,10 +107,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
   int k2 = dig[2];
   int top = Np - 1;   // recompute nodes top..3
   bool need_heavy = true;
-  constexpr bool kCtxShared = L >= 6;   // many levels: the node-2 context does not fit the register file beside the tables
+  constexpr bool kCtxShared = L >= CTX_SHARED_MIN_L;   // many levels: the node-2 context does not fit the register file beside the tables
   float D3[NBX];
   float X2r[L], Rm3r[L], U1rr[L], A0rr[L];   // node-2 context in registers (L < 6)
-  float* cx = ws->ctx + lane;                 // this lane's column of the node-2 context in shared memory (L >= 6)
+  float4* cx = ws->ctx + lane;                // this lane's column of the node-2 context in shared memory
   float C3 = 0.0f;
   float nthrm[L];   // -pred(thr_l): the screen's addend
   // lane l < Lr reads the bits of the best C the request's warps have published for level l, one light step ahead
@@ -161,7 +167,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
     for (int l = 0; l < L; l++) {
       if (kCtxShared) {
-        cx[(4 * l + 0) * 32] = X2[l]; cx[(4 * l + 1) * 32] = Rm[3][l]; cx[(4 * l + 2) * 32] = U1r[l]; cx[(4 * l + 3) * 32] = A0r[l];
+        cx[l * 32] = make_float4(X2[l], Rm[3][l], U1r[l], A0r[l]);
       } else {
         X2r[l] = X2[l]; Rm3r[l] = Rm[3][l]; U1rr[l] = U1r[l]; A0rr[l] = A0r[l];
       }
@@ -189,10 +195,12 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     float R2[L], U1pS[L], A0q1[L];
 #pragma unroll
     for (int l = 0; l < L; l++) {
-      const float u2 = (kCtxShared ? cx[(4 * l + 0) * 32] : X2r[l]) + s_nlat[slot2 * L + l];
-      R2[l] = fminf(kCtxShared ? cx[(4 * l + 1) * 32] : Rm3r[l], u2);
-      const float U1 = fminf(kCtxShared ? cx[(4 * l + 2) * 32] : U1rr[l], u2 + big12);
-      const float a0 = fminf(kCtxShared ? cx[(4 * l + 3) * 32] : A0rr[l], u2 + big02);
+      float4 c4;
+      if (kCtxShared) c4 = cx[l * 32]; else c4 = make_float4(X2r[l], Rm3r[l], U1rr[l], A0rr[l]);
+      const float u2 = c4.x + s_nlat[slot2 * L + l];
+      R2[l] = fminf(c4.y, u2);
+      const float U1 = fminf(c4.z, u2 + big12);
+      const float a0 = fminf(c4.w, u2 + big02);
       A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
       U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
     }
