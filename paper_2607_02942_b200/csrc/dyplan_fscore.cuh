@@ -264,7 +264,11 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
           for (int b = 0; b < NBX; b++) ws->scr[kScrS1 + b] = NB ? sD2[b] : 0.0f;
 #pragma unroll
-          for (int l = 0; l < L; l++) { ws->scr[kScrAp1 + l] = A0q1[l]; ws->scr[kScrU1 + l] = U1pS[l]; ws->scr[kScrR2 + l] = R2[l]; }
+          for (int l = 0; l < L; l++) {
+            ws->scr[kScrAp1 + l] = A0q1[l]; ws->scr[kScrU1 + l] = U1pS[l];
+            // R2 is only needed here: with the context in shared memory it is re-derived instead of being kept live
+            ws->scr[kScrR2 + l] = kCtxShared ? fminf(cx[l * 32].y, cx[l * 32].x + s_nlat[slot2 * L + l]) : R2[l];
+          }
         }
         __syncwarp();
         const float gC2 = ws->scr[kScrC1];
