@@ -31,9 +31,9 @@ METRIC = "plan_level_evaluations_per_s"
 UNIT = "Geval/s"
 SM_LANES = 128            # FP32/INT32 lanes per SM = 4 SMSPs x 32 (one warp instruction per clock per SMSP)
 # dram__bytes_read.sum + dram__bytes_write.sum of the scoring kernel, per launch, from the `ncu --set full` captures of
-# profiles/r1e_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
+# profiles/r1f_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
 # (cfg4's is local-memory write-back).  None for a workload that was not captured (cfg0, down-scaled runs).
-NCU_DRAM_BYTES = {1: 25.74e6, 2: 49.58e6, 3: 96.25e6, 4: 393.49e6}
+NCU_DRAM_BYTES = {1: 11.11e6, 2: 30.37e6, 3: 92.66e6, 4: 236.57e6}
 
 
 def alg_ops_per_eval(w) -> float:
