@@ -112,7 +112,14 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
   float X2r[L], Rm3r[L], U1rr[L], A0rr[L];   // node-2 context in registers (L < 6)
   float4* cx = ws->ctx + lane;                // this lane's column of the node-2 context in shared memory
   float C3 = 0.0f;
-  float nthrm[L];   // -pred(thr_l): the screen's addend
+  // Two forms of the screen's incumbent test, same decision up to false positives the slow path rejects:
+  //   product form   z = x * (C1 * f0[k0]) - pred(thr_l)            one FMUL per plan
+  //   quotient form  z = x * f0[k0] - pred(thr_l) (1 - 2^-20) / C1  one reciprocal and L FMULs per group, none per plan;
+  //                  taken when node 0 has more options than that costs.  fl(C1 f0) >= thr implies
+  //                  f0 >= thr / (C1 (1 + 2^-24)) > the addend above (reciprocal and products err by < 2^-22), so no
+  //                  plan that ties or beats the incumbent is screened out; plans within 1e-6 of it may pass.
+  constexpr bool kQuot = K0P >= L + 8;   // (measured: no gain at 8 options x 4 levels, 3 % at 12 x 1)
+  float nthrm[L];   // -pred(thr_l) (times 1 - 2^-20 in the quotient form): the screen's addend
   // lane l < Lr reads the bits of the best C the request's warps have published for level l, one light step ahead
   const int* gaddr = g_thr + (lane < Lr ? lane : 0);
   asm volatile("" : "+l"(gaddr));   // keep the address in its own register pair (not rematerialised into a scratch pair)
@@ -184,7 +191,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) {
         const int t = max(((volatile int*)w_thr)[l], __shfl_sync(0xffffffffu, gpub, l));
-        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
+        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000) * (kQuot ? 0.99999905f : 1.0f);
       }
       gpub = __ldcg(gaddr);
     }
@@ -230,13 +237,23 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
       float zodd = 0.0f;             // odd L: the last level of an even k0 waits for the one of k0 + 1 (one FMNMX3 for both)
+      float addend[L];
+      if (kQuot) {
+        float rc;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(C1));
+#pragma unroll
+        for (int l = 0; l < L; l++) addend[l] = (NB && !(C1 > 0.0f)) ? -4.0f : nthrm[l] * rc;   // (C1 = 0: a cap is already exceeded)
+      } else {
+#pragma unroll
+        for (int l = 0; l < L; l++) addend[l] = nthrm[l];
+      }
 #pragma unroll
       for (int k0 = 0; k0 < K0P; k0++) {
-        float P = C1 * f0[k0];
+        float P = kQuot ? f0[k0] : C1 * f0[k0];
         if (NB) P *= __saturatef(s1[k0 / G] + ndem0[k0]);
         float z[L];
 #pragma unroll
-        for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, nthrm[l]);
+        for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, addend[l]);
 #pragma unroll
         for (int l = 0; l + 1 < L; l += 2) {
           if (NB && (((l >> 1) + k0) & 1)) zm2 = fmaxf(zm2, fmaxf(z[l], z[l + 1]));
@@ -346,7 +363,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) {
         const int t = ((volatile int*)w_thr)[l];
-        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000);
+        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000) * (kQuot ? 0.99999905f : 1.0f);
       }
     }
     // ---- advance ----
