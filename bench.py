@@ -33,7 +33,7 @@ SM_LANES = 128            # FP32/INT32 lanes per SM = 4 SMSPs x 32 (one warp ins
 # dram__bytes_read.sum + dram__bytes_write.sum of the scoring kernel, per launch, from the `ncu --set full` captures of
 # profiles/r1f_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
 # (cfg4's is local-memory write-back).  None for a workload that was not captured (cfg0, down-scaled runs).
-NCU_DRAM_BYTES = {1: 11.11e6, 2: 30.37e6, 3: 92.66e6, 4: 236.57e6}
+NCU_DRAM_BYTES = {1: 10.95e6, 2: 33.23e6, 3: 93.20e6, 4: 253.69e6}
 
 
 def alg_ops_per_eval(w) -> float:
