@@ -164,3 +164,30 @@ def test_linear_argument_errors(dy):
     with pytest.raises(binding.DyplanError) as e:
         ctx.dyplan_compile_linear(db, None, P0, [0.0], out)
     assert e.value.code == binding.ERR_NULL
+
+
+def test_linear_full_size_cfg1_shapes(dy):
+    """The configuration bench.py --objective linear times (256 requests x 8^8 plans x 3 levels): every record re-scored by
+    the oracle (T, D_tau bit-identical, J64 within 1e-12), full brute force on two sampled requests."""
+    from oracle import linear as lo
+    w = wl.make_config(1)
+    cost = np.random.default_rng(7).uniform(0.0, 1.0, size=w.batch.lat_us.size).astype(np.float32)
+    p = f32(dict(lambda_f=0.5, lambda_c=0.1, lambda_l=0.0002, lambda_ld=0.0001, beta=0.5, effort=1.0))
+    levels = [0.0, 1.5, 3.0]
+    g, st = run_gpu(dy, w.batch, cost, p, levels)
+    assert st["plans"] == 256 * 8**8 and (g["status"] == 0).all()
+    ch = g["choice"].reshape(-1, 16)
+    for rec in range(256 * 3):
+        r, l = divmod(rec, 3)
+        s = lo.score(w.batch, cost, p, r, levels[l], ch[rec].copy())
+        assert s["status"] == 0 and s["T"] == int(g["lat"][rec]) and s["Dtau"] == int(g["dtau"][rec]), rec
+        assert abs(s["J"] - float(g["corr64"][rec])) <= 1e-12 * max(1.0, abs(s["J"])), rec
+    assert (np.diff(g["dtau"].reshape(256, 3), axis=1) <= 0).all()          # PAPER.md:207
+    rows = [17, 200]
+    sub = w.subset(rows)
+    o0 = [int(w.batch.opt_off[int(w.batch.node_off[r])]) for r in rows]
+    o1 = [int(w.batch.opt_off[int(w.batch.node_off[r + 1])]) for r in rows]
+    csub = np.concatenate([cost[a:b] for a, b in zip(o0, o1)])
+    ref = lo.compile(sub.batch, csub, p, levels)
+    gs = {k: v.reshape(256, -1)[rows].reshape(-1) for k, v in g.items()}
+    check(lo, sub.batch, csub, p, levels, gs, ref)
