@@ -238,7 +238,8 @@ DYPLAN_API int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, co
                           const dyplan_linear_params* params, int32_t L, const float* levels, dyplan_bundle* out,
                           const dyplan_linear_extra* extra, void* stream);
 
-/* Same three calls with HOST pointers everywhere (batch fields, multipliers, masks, outputs).  The library copies
+/* The compile / replan / select / compile_linear calls with HOST pointers everywhere (batch fields, multipliers, masks,
+ * cost, outputs, extras).  The library copies
  * inputs to the device, runs the same kernels and copies the results back, all on `stream`, and returns after a
  * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied. */
 DYPLAN_API int dyplan_compile_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
@@ -246,6 +247,9 @@ DYPLAN_API int dyplan_compile_host(dyplan_ctx* ctx, const dyplan_batch* in, int3
 DYPLAN_API int dyplan_replan_host(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask,
                        const uint8_t* fixed_choice, const int32_t* live_mult_pm, uint32_t flags, dyplan_bundle* out,
                        void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+DYPLAN_API int dyplan_compile_linear_host(dyplan_ctx* ctx, const dyplan_batch* in, const float* cost,
+                               const dyplan_linear_params* params, int32_t L, const float* levels, dyplan_bundle* out,
+                               const dyplan_linear_extra* extra, void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 DYPLAN_API int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L,
                        const int32_t* live_mult_pm, int32_t* variant, dyplan_bundle* rescored, void* stream,
                        uint64_t* h2d_bytes, uint64_t* d2h_bytes);

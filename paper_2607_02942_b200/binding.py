@@ -26,7 +26,7 @@ FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
 EXPORTS = (
-    "dyplan_create", "dyplan_destroy", "dyplan_set_flags", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_bind",
+    "dyplan_create", "dyplan_destroy", "dyplan_set_flags", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_compile_linear_host", "dyplan_bind",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
 )
@@ -97,6 +97,7 @@ def lib():
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
         l.dyplan_compile_linear.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp]
+        l.dyplan_compile_linear_host.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp, pu64, pu64]
         l.dyplan_bind.argtypes = [vp, C.POINTER(CProfiles), i32, i32] + [vp] * 13
         l.dyplan_switch.argtypes = [vp, pb, po, i32, C.POINTER(CSwitchParams), vp, vp, vp, vp, vp, vp, vp]
         l.dyplan_compile_host.argtypes = [vp, pb, i32, vp, po, vp, pu64, pu64]
@@ -299,6 +300,17 @@ class Context:
         self._check(lib().dyplan_bind(self._h, C.byref(p), NN, KK, _ptr(opt_off), _ptr(pred_mask), _ptr(skill), _ptr(role),
                                       _ptr(model), _ptr(backend), _ptr(policy), _ptr(vuln), _ptr(acc), _ptr(lat_us),
                                       _ptr(cost), _ptr(demand), _stream_ptr(stream)))
+
+    def dyplan_compile_linear_host(self, batch: Buffers, cost: np.ndarray, params: dict, levels, out: Buffers, dtau=None,
+                                   quality=None, stream=None):
+        p = CLinearParams(*[float(params[n]) for n, _ in CLinearParams._fields_])
+        lv = np.ascontiguousarray(levels, np.float32)
+        ex = CLinearExtra(_ptr(dtau), _ptr(quality))
+        h2d, d2h = C.c_uint64(), C.c_uint64()
+        self._check(lib().dyplan_compile_linear_host(self._h, C.byref(batch.cstruct), _ptr(cost), C.byref(p), int(lv.size),
+                                                     lv.ctypes.data_as(C.c_void_p), C.byref(out.cstruct), C.byref(ex),
+                                                     _stream_ptr(stream), C.byref(h2d), C.byref(d2h)))
+        return h2d.value, d2h.value
 
     def dyplan_set_flags(self, flags: int):
         self._check(lib().dyplan_set_flags(self._h, int(flags)))

@@ -441,6 +441,7 @@ size_t arena_bytes(const HostPlan& p) {
     add(p.nrec * 8); add(p.nrec * 16); add(p.nrec * 4); add(p.nrec * 8); add(p.nrec * 4); add(p.nrec * p.B * 4); add(p.nrec); add(p.nrec);
   }
   add(p.R * 4);
+  add(p.KK * 4); add(p.nrec * 4); add(p.nrec * 8);   // linear mode: cost, dtau, quality
   return n;
 }
 
@@ -548,6 +549,43 @@ int dyplan_replan_host(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* 
                        uint64_t* d2h_bytes) {
   if (flags & ~DYPLAN_RESIDUAL) return DYPLAN_ERR_ARG;
   return solve_host(ctx, in, 1, live_mult_pm, dispatched_mask, fixed_choice, flags, true, out, stream, h2d_bytes, d2h_bytes);
+}
+
+int dyplan_compile_linear_host(dyplan_ctx* ctx, const dyplan_batch* in, const float* cost, const dyplan_linear_params* params, int32_t L,
+                               const float* levels, dyplan_bundle* out, const dyplan_linear_extra* extra, void* stream,
+                               uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  int rc = host_sizes_ok(in);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  uint64_t h2d = 0, d2h = 0;
+  if (h2d_bytes) *h2d_bytes = 0;
+  if (d2h_bytes) *d2h_bytes = 0;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!params || !levels || (in->KK > 0 && !cost)) return DYPLAN_ERR_NULL;
+  if ((rc = check_bundle(out))) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  HostPlan hp{(size_t)in->R, (size_t)in->NN, (size_t)in->KK, (size_t)in->B, (size_t)L, (size_t)in->R * L};
+  if ((rc = ensure(ctx, ctx->arena, arena_bytes(hp)))) return rc;
+  Arena ar{(char*)ctx->arena.p, 0};
+  dyplan_batch d;
+  if ((rc = batch_to_device(ctx, in, ar, &d, s, h2d))) return rc;
+  float* dcost;
+  H2D(dcost, cost, (size_t)in->KK, float);
+  dyplan_bundle dout;
+  bundle_alloc(ar, hp.nrec, hp.B, out->corr64 != nullptr, &dout);
+  dyplan_linear_extra dex;
+  dex.dtau = (extra && extra->dtau) ? ar.take<int32_t>(hp.nrec) : nullptr;
+  dex.quality = (extra && extra->quality) ? ar.take<double>(hp.nrec) : nullptr;
+  if ((rc = dyplan_compile_linear(ctx, &d, dcost, params, L, levels, &dout, &dex, stream))) return rc;
+  if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h))) return rc;
+  if (dex.dtau) D2H(extra->dtau, dex.dtau, hp.nrec, int32_t);
+  if (dex.quality) D2H(extra->quality, dex.quality, hp.nrec, double);
+  CK(cudaStreamSynchronize(s));
+  if (h2d_bytes) *h2d_bytes = h2d;
+  if (d2h_bytes) *d2h_bytes = d2h;
+  return DYPLAN_OK;
 }
 
 int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bundle* bundle, int32_t L, const int32_t* live_mult_pm,

@@ -166,6 +166,27 @@ def test_linear_argument_errors(dy):
     assert e.value.code == binding.ERR_NULL
 
 
+def test_linear_host_call_matches_device_call(dy):
+    binding, ctx = dy
+    batch, cost = case(206, R=24, nmin=1, nmax=7, kmin=1, kmax=6)
+    p, levels = f32(P0), [0.0, 1.0, 4.0]
+    g, _ = run_gpu(dy, batch, cost, p, levels)
+    hb = binding.make_batch(batch, None)
+    hout = binding.alloc_bundle(batch.R, 3, batch.B, None, True)
+    dtau = np.full(batch.R * 3, -5, np.int32)
+    qual = np.full(batch.R * 3, -5.0, np.float64)
+    h2d, d2h = ctx.dyplan_compile_linear_host(hb, cost, p, levels, hout, dtau, qual)
+    h = hout.host()
+    for k in ("status", "plan_idx", "choice", "lat", "corr", "corr64", "dem", "dom_model"):
+        assert np.array_equal(h[k], g[k]), k
+    assert np.array_equal(dtau, g["dtau"]) and np.array_equal(qual, g["quality"])
+    assert h2d >= cost.nbytes + batch.lat_us.nbytes and d2h >= h["plan_idx"].nbytes + dtau.nbytes + qual.nbytes
+    # extras are optional; an empty batch is a no-op
+    hout2 = binding.alloc_bundle(batch.R, 3, batch.B, None, False)
+    ctx.dyplan_compile_linear_host(hb, cost, p, levels, hout2)
+    assert np.array_equal(hout2.host()["plan_idx"], g["plan_idx"])
+
+
 def test_linear_full_size_cfg1_shapes(dy):
     """The configuration bench.py --objective linear times (256 requests x 8^8 plans x 3 levels): every record re-scored by
     the oracle (T, D_tau bit-identical, J64 within 1e-12), full brute force on two sampled requests."""
