@@ -188,11 +188,11 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     {
       // thresholds: this warp's, raised by what the other warps of the request had published one light step ago
       // (the load issued here is consumed at the next step, which keeps its L2 latency off the critical path)
+      // (lane l derives level l's addend, the warp reads it by shuffle: one max/decrement/negate instead of L)
+      const int t = max(((volatile int*)w_thr)[lane & 7], gpub);
+      const float nv = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000) * (kQuot ? 0.99999905f : 1.0f);
 #pragma unroll
-      for (int l = 0; l < L; l++) {
-        const int t = max(((volatile int*)w_thr)[l], __shfl_sync(0xffffffffu, gpub, l));
-        nthrm[l] = __int_as_float((t > 0 ? t - 1 : 0) | (int)0x80000000) * (kQuot ? 0.99999905f : 1.0f);
-      }
+      for (int l = 0; l < L; l++) nthrm[l] = __shfl_sync(0xffffffffu, nv, l);
       gpub = __ldcg(gaddr);
     }
 
