@@ -115,6 +115,15 @@ typedef struct {
  *   changes is dyplan_stats.plans, which then counts the plans of the pruned space, and the 2^40 limit, which applies
  *   to the pruned space.  Applies to requests the fp32 scorer takes; others are enumerated in full. */
 #define DYPLAN_PRUNE_DOMINATED 1u
+/* DYPLAN_PRUNE_BOUNDS: while enumerating, skip a whole subtree (all options of the three innermost enumeration digits
+ *   below one assignment of the outer nodes) when no plan in it can replace an incumbent: the outer nodes' demand
+ *   already exceeds a cap, or at every level either a node misses the SLO even with the shortest options of the inner
+ *   nodes (a latency lower bound: durations are >= 0, so the longest path only grows), or the separable upper bound on
+ *   C -- the outer nodes' product times the largest factor of each inner node, rounded as the scorer rounds -- is
+ *   below the best C already found for that level (second half).
+ *   Exact: results are those of the full enumeration (parity-tested against the unpruned oracle).  dyplan_stats.plans
+ *   still counts the whole space; dyplan_stats.bound_skipped counts the outer indices that were not walked. */
+#define DYPLAN_PRUNE_BOUNDS 2u
 
 /* Create / destroy a context on CUDA device `device_ordinal`.  Fails (DYPLAN_ERR_CUDA) without a device. */
 DYPLAN_API int dyplan_create(dyplan_ctx** out, int device_ordinal);
@@ -264,6 +273,7 @@ typedef struct {
   int32_t launches;     /* kernels launched by the last call                                                      */
   int32_t sm_count;     /* SMs of the device                                                                      */
   float score_ms;       /* device time of the scoring kernel of the last call (CUDA events on `stream`)           */
+  uint64_t bound_skipped; /* outer indices (assignments of all but the two innermost digits) skipped by DYPLAN_PRUNE_BOUNDS */
 } dyplan_stats;
 /* Synchronises `stream` of the last call, then fills *out. */
 DYPLAN_API int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out);

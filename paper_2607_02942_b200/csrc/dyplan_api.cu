@@ -140,7 +140,7 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
 
 int dyplan_set_flags(dyplan_ctx* ctx, uint32_t flags) {
   if (!ctx) return DYPLAN_ERR_NULL;
-  if (flags & ~DYPLAN_PRUNE_DOMINATED) return DYPLAN_ERR_ARG;
+  if (flags & ~(DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS)) return DYPLAN_ERR_ARG;
   ctx->flags = flags;
   return DYPLAN_OK;
 }
@@ -400,6 +400,7 @@ int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
     out->work_items = (uint64_t)st.total_items + st.total_items_f;
     out->fast_requests = st.fast_requests;
     out->slow_steps = st.slow_steps;
+    out->bound_skipped = st.bound_skipped;
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     out->score_ms = ms;

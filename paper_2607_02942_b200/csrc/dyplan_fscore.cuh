@@ -26,7 +26,8 @@ struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
   Best best[8];                    // the warp's incumbent per level (written by the cooperative slow path only)
   int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
-  float scr[40];                   // slow path: the flagged lane's group state, broadcast through shared memory
+  float scr[68];                   // slow path: the flagged lane's group state, broadcast through shared memory;
+                                   // [36..64]: subtree bounds (DYPLAN_PRUNE_BOUNDS), written once per work item
   float4 ctx[(L >= CTX_SHARED_MIN_L ? L * 32 : 1)];   // (L >= CTX_SHARED_MIN_L) [l][lane] = {X2, Rm3, U1r, A0r}: node-2 context of every lane, written
                                    // by the heavy step and read by each light step (kept out of the register file)
   unsigned long long bar;          // mbarrier of the TMA copy
@@ -38,6 +39,8 @@ struct __align__(16) FWarpShared {
 #endif
 // scratch layout of the cooperative slow path
 constexpr int kScrC1 = 0, kScrS1 = 1, kScrAp1 = 9, kScrU1 = 17, kScrR2 = 25, kScrIdx = 34;
+// subtree bounds: on/off, largest factor of nodes 2, 1, 0, number of (lane, node-2 sweep) pairs skipped in this item
+constexpr int kScrBnd = 36, kScrF2 = 37, kScrF1 = 38, kScrF0 = 39, kScrSkip = 40, kScrMx = 44;   // kScrMx: [node 2, 1, 0][8 levels]
 
 // Loop nest of one lane over `steps` outer indices (digits of internal nodes >= 2, odometer order).  Every lane of
 // the warp runs the same number of steps (a lane whose own range is shorter keeps walking with C = 0, which can
@@ -152,7 +155,30 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
         for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0.0f);
       }
     }
-    {
+    // ---- subtree bound (DYPLAN_PRUNE_BOUNDS; items whose lanes are in phase, so these branches are warp-uniform) ----
+    // Every plan below this prefix has C32 <= ub (rounding is monotone and the factors are taken in the scorer's
+    // order); it misses the SLO at level l if a node >= 3 already does, and breaks a cap if the outer nodes' demand
+    // already does.  The slow path admits a plan only with C32 >= thr_l, so a prefix that is dead at every level, in
+    // every lane, cannot change an incumbent.
+    const bool bnd = ws->scr[kScrBnd] != 0.0f;
+    bool bskip = false;
+    unsigned lvl_alive = 0u;
+    if (bnd) {
+      const float ub = __fmul_rn(__fmul_rn(__fmul_rn(Cp[3], ws->scr[kScrF2]), ws->scr[kScrF1]), ws->scr[kScrF0]);
+      const int tmine = max(((volatile int*)w_thr)[lane & 7], gpub);
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const int tl = __shfl_sync(0xffffffffu, tmine, l);
+        if (Rm[3][l] >= 0.0f && ub >= __int_as_float(tl)) lvl_alive |= 1u << l;
+      }
+      if (NB) {
+#pragma unroll
+        for (int b = 0; b < NBX; b++) if (!(Dp[3][b] <= capf[b])) lvl_alive = 0u;
+      }
+      if (!(step < my_count)) lvl_alive = 0u;
+      bskip = !__any_sync(0xffffffffu, lvl_alive != 0u);
+    }
+    if (!bskip) {
     float X2[L], U1r[L], A0r[L];
 #pragma unroll
     for (int l = 0; l < L; l++) { X2[l] = slo; U1r[l] = slo; A0r[l] = slo; }
@@ -171,6 +197,18 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) A0r[l] = fminf(A0r[l], u[j][l]);
     }
+    if (bnd) {
+      // second test, with the context just built: node 2, 1 or 0 misses the SLO even with its shortest option behind
+      // the outer nodes alone (X2, U1r, A0r only shrink when inner predecessors are added)
+      bool alive = false;
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        const float* mx = &ws->scr[kScrMx + l];   // largest negated duration of nodes 2, 1, 0 at level l
+        alive = alive || (((lvl_alive >> l) & 1u) && X2[l] + mx[0] >= 0.0f && U1r[l] + mx[8] >= 0.0f && A0r[l] + mx[16] >= 0.0f);
+      }
+      bskip = !__any_sync(0xffffffffu, alive);
+    }
+    if (!bskip) {
 #pragma unroll
     for (int l = 0; l < L; l++) {
       if (kCtxShared) {
@@ -179,6 +217,23 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
         X2r[l] = X2[l]; Rm3r[l] = Rm[3][l]; U1rr[l] = U1r[l]; A0rr[l] = A0r[l];
       }
     }
+    }
+    }
+    if (bskip) {
+      // no lane of the warp can change an incumbent below this prefix: skip node 2's whole sweep
+      const unsigned nlive = __popc(__ballot_sync(0xffffffffu, step < my_count));
+      if (lane == 0) ((unsigned*)ws->scr)[kScrSkip] += nlive;
+      step += (unsigned long long)(K2 - 1);
+      gpub = __ldcg(gaddr);   // keep following what the other warps publish while skipping
+      int i = 3;
+      for (; i < Np; i++) {
+        const int d = dig[i] + 1;
+        if (d < h->Kp[i]) { dig[i] = (unsigned char)d; break; }
+        dig[i] = 0;
+      }
+      top = i < Np ? i : Np - 1;
+      need_heavy = true;
+      continue;
     }
     C3 = Cp[3];
 #pragma unroll
@@ -440,6 +495,31 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     const unsigned long long tb = min(ob + (unsigned long long)lane * per, oe);
     const unsigned long long te = min(tb + per, oe);
     {
+      // subtree bounds: only when every lane starts a sweep of node 2 at the same step (the bound test votes warp-wide)
+      const bool bnd = (a.ctx_flags & DYPLAN_PRUNE_BOUNDS) && ob % K2u == 0 && per % K2u == 0;
+      if (lane == 0) {
+        ws->scr[kScrBnd] = bnd ? 1.0f : 0.0f;
+        ((unsigned*)ws->scr)[kScrSkip] = 0u;
+        if (bnd) {
+          const float* sf = (const float*)(ws->blob + kHdrWords) + h->nslots_pad * L;
+          float m2 = 0.0f, m1 = 0.0f, m0 = 0.0f;
+          for (int k = 0; k < h->Kp[2]; k++) m2 = fmaxf(m2, sf[h->optbase[2] + k]);
+          for (int k = 0; k < h->K1; k++) m1 = fmaxf(m1, sf[h->K0p + k]);
+          for (int k = 0; k < h->K0p; k++) m0 = fmaxf(m0, sf[k]);
+          ws->scr[kScrF2] = m2; ws->scr[kScrF1] = m1; ws->scr[kScrF0] = m0;
+          const float* sl = (const float*)(ws->blob + kHdrWords);   // [slot][L] negated durations
+          for (int l = 0; l < L; l++) {
+            float x2 = -kBigF, x1 = -kBigF, x0 = -kBigF;
+            for (int k = 0; k < h->Kp[2]; k++) x2 = fmaxf(x2, sl[(h->optbase[2] + k) * L + l]);
+            for (int k = 0; k < h->K1; k++) x1 = fmaxf(x1, sl[(h->K0p + k) * L + l]);
+            for (int k = 0; k < h->K0p; k++) x0 = fmaxf(x0, sl[k * L + l]);   // (padding slots hold -2^25: never the maximum)
+            ws->scr[kScrMx + l] = x2; ws->scr[kScrMx + 8 + l] = x1; ws->scr[kScrMx + 16 + l] = x0;
+          }
+        }
+      }
+      __syncwarp();
+    }
+    {
       const unsigned long long n = te - tb;
       const unsigned long long t0 = n ? tb : 0ull;   // an idle lane walks from outer index 0 (with C = 0)
       switch (h->nbc * 32 + h->K0p) {
@@ -454,6 +534,8 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
       }
     }
     __syncwarp();
+    if (lane == 0 && ((const unsigned*)ws->scr)[kScrSkip])
+      atomicAdd(&a.st->bound_skipped, (unsigned long long)((const unsigned*)ws->scr)[kScrSkip] * K2u);
     // ---- the warp's incumbents are the item's records; lane l keeps level l ----
     Best mine; mine.C = -1.0f; mine.T = INT32_MAX; mine.idx = kNoIdx;
     if (lane < Lr) mine = ws->best[lane];

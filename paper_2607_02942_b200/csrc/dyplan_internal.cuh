@@ -81,6 +81,7 @@ struct CallState {
   unsigned long long per_item_outer;   // wide class: outer indices per (block) work item
   unsigned long long per_item_outer_f; // fast class: outer indices per (warp) work item
   unsigned long long slow_steps;
+  unsigned long long bound_skipped;    // outer indices the subtree bound skipped (DYPLAN_PRUNE_BOUNDS)
   uint32_t total_items;             // wide class
   uint32_t next_item;               // wide class: dynamic work counter
   uint32_t total_items_f;           // fast class
@@ -97,7 +98,7 @@ struct CallArgs {                   // passed by value to the kernels
   const uint32_t* dispatched;       // replan only
   const uint8_t* fixed_choice;      // replan only
   uint32_t flags;
-  uint32_t ctx_flags;               // DYPLAN_PRUNE_DOMINATED (dyplan_set_flags)
+  uint32_t ctx_flags;               // DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS (dyplan_set_flags)
   int32_t is_replan;
   // scratch
   uint32_t* blob;                   // staged requests

@@ -551,7 +551,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     a.item_off_f[R] = total_items_f;
     CallState* st = a.st;
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
-    st->slow_steps = 0;
+    st->slow_steps = 0; st->bound_skipped = 0;
     st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
     st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u;
   }

@@ -494,3 +494,85 @@ def test_pruning_reaches_a_space_beyond_brute_force(dy, orc, pruning):
     ctx.dyplan_set_flags(0)
     g0 = gpu_run(dy, w)
     assert (g0["status"] == 3).all()                             # the same batch without pruning: plan space too large
+
+
+# ---- exact subtree bounds (second half): same results, fewer plans walked ----------
+@pytest.fixture()
+def bounding(dy):
+    binding, ctx = dy
+    ctx.dyplan_set_flags(binding.PRUNE_BOUNDS)
+    yield
+    ctx.dyplan_set_flags(0)
+
+
+@pytest.mark.parametrize("seed,L,B,caps", [(131, 1, 1, False), (132, 3, 2, True), (133, 4, 3, True), (134, 8, 2, False),
+                                           (135, 6, 2, True), (136, 2, 1, False)])
+def test_bounded_enumeration_equals_the_full_oracle(dy, orc, bounding, seed, L, B, caps):
+    w = wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=8, B=B, M=3, L=L, caps=caps)
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    assert st["plans"] == w.n_plans_total()                     # the space is the whole space ...
+    check_records(orc, w, g, orc.run(w), where=f"bounded(seed={seed})")   # ... and nothing changed
+
+
+def test_bounded_configs_skip_subtrees_and_change_nothing(dy, orc, bounding):
+    # large enough for lane-aligned work items (the bound votes warp-wide and is off for calls too small to fill the GPU)
+    binding, ctx = dy
+    for w in (wl.make_config(1, R=16), wl.make_config(2, R=96), wl.make_config(3, R=64)):
+        g = gpu_run(dy, w)
+        st = ctx.dyplan_last_stats()
+        check_records(orc, w, g, orc.run(w), where=f"bounded {w.name}")
+        assert st["bound_skipped"] > 0, w.name                  # the bound did cut something on the paper-shaped inputs
+        assert st["plans"] == w.n_plans_total()
+    for w in (wl.make_config(0), wl.make_config(1, R=2), wl.make_config(4, R=1)):   # small calls: bound off or on, same records
+        if w.name.startswith("cfg4"):
+            w.batch.slo_us[:] //= 3                              # mostly infeasible prefixes: the latency bound cuts
+            ctx.dyplan_set_flags(0)
+            ref = gpu_run(dy, w)                                 # 6^12 plans: the exhaustive GPU run is the comparison
+            ctx.dyplan_set_flags(binding.PRUNE_BOUNDS)
+            g = gpu_run(dy, w)
+            for k in ("plan_idx", "lat", "dem", "status", "choice", "corr"):
+                assert np.array_equal(g[k], ref[k]), k
+        else:
+            check_records(orc, w, gpu_run(dy, w), orc.run(w), where=f"bounded {w.name}")
+
+
+def test_bounded_random_batches_large_enough_to_align(dy, orc, bounding):
+    for seed, L, B, caps in [(141, 3, 2, True), (142, 2, 3, False)]:
+        w = wl.random_workload(seed, R=300, nmin=6, nmax=7, kmin=5, kmax=8, B=B, M=3, L=L, caps=caps)
+        g = gpu_run(dy, w)
+        st = dy[1].dyplan_last_stats()
+        check_records(orc, w, g, orc.run(w), where=f"bounded aligned(seed={seed})")
+        assert st["bound_skipped"] > 0
+    w = wl.random_replan_workload(137, R=40, nmin=1, nmax=8, kmin=1, kmax=6, B=3, M=3, caps=True)
+    check_records(orc, w, gpu_run(dy, w), orc.run(w), where="bounded replan")
+    w.flags = wl.FLAG_RESIDUAL
+    check_records(orc, w, gpu_run(dy, w), orc.run(w), where="bounded replan residual")
+
+
+def test_bounds_with_exact_ties_keep_the_tie_break(dy, orc, bounding):
+    # many plans tie with the optimum in C: a subtree whose bound EQUALS the incumbent must still be walked (T, idx decide)
+    w = wl.make_config(1, R=12)
+    b = w.batch
+    b.acc[:] = np.round(b.acc * 4) / 4
+    b.vuln[:] = np.round(b.vuln * 2) / 2
+    b.lat_us[:] = (b.lat_us // 400 + 1) * 400
+    g = gpu_run(dy, w)
+    ref = orc.run(w)
+    check_records(orc, w, g, ref, where="bounded ties")
+    ok = ref["status"] == 0
+    assert (g["plan_idx"][ok] == ref["plan_idx"][ok]).all()
+
+
+def test_bounds_and_dominance_pruning_together(dy, orc):
+    binding, ctx = dy
+    ctx.dyplan_set_flags(binding.PRUNE_BOUNDS | binding.PRUNE_DOMINATED)
+    try:
+        for seed, L, B, caps in [(138, 4, 2, True), (139, 3, 3, False)]:
+            w = wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=8, B=B, M=3, L=L, caps=caps)
+            check_records(orc, w, gpu_run(dy, w), orc.run(w), where=f"bounded+pruned(seed={seed})")
+        with pytest.raises(binding.DyplanError) as e:
+            ctx.dyplan_set_flags(4)                              # unknown bit
+        assert e.value.code == binding.ERR_ARG
+    finally:
+        ctx.dyplan_set_flags(0)
