@@ -31,9 +31,9 @@ METRIC = "plan_level_evaluations_per_s"
 UNIT = "Geval/s"
 SM_LANES = 128            # FP32/INT32 lanes per SM = 4 SMSPs x 32 (one warp instruction per clock per SMSP)
 # dram__bytes_read.sum + dram__bytes_write.sum of the scoring kernel, per launch, from the `ncu --set full` captures of
-# profiles/r1f_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
+# profiles/r1g_k_fscore.md (bytes).  The kernel is issue-bound; this is reported to show the traffic is negligible
 # (cfg4's is local-memory write-back).  None for a workload that was not captured (cfg0, down-scaled runs).
-NCU_DRAM_BYTES = {1: 10.95e6, 2: 33.23e6, 3: 93.20e6, 4: 253.69e6}
+NCU_DRAM_BYTES = {1: 13.85e6, 2: 33.97e6, 3: 94.34e6, 4: 232.98e6}
 
 
 def alg_ops_per_eval(w) -> float:
@@ -181,6 +181,10 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
     ctx = binding.Context(local_rank)
+    prune_flags = {"none": 0, "dominated": binding.PRUNE_DOMINATED, "bounds": binding.PRUNE_BOUNDS,
+                   "both": binding.PRUNE_DOMINATED | binding.PRUNE_BOUNDS}[args.prune]
+    if prune_flags:
+        ctx.dyplan_set_flags(prune_flags)
     w = make_workload(args.config, rank, args.requests)
     dw = binding.upload(w, dev, corr64=True)
     stream = torch.cuda.Stream(device=dev)
@@ -198,7 +202,8 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
             binding.launch(ctx, dw, stream)
         stream.synchronize()
         st = ctx.dyplan_last_stats()
-        assert st["plans"] == plans, (st, plans)
+        # dominance pruning shrinks the enumerated space; stats report the plans actually enumerated
+        assert st["plans"] == plans or (prune_flags & binding.PRUNE_DOMINATED and st["plans"] <= plans), (st, plans)
         launches_per_step = st["launches"]
         sampler = ClockSampler(local_rank)
         barrier()
@@ -296,6 +301,13 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
                      "ops_per_eval": aops, "kernel_ms": k_ms / args.steps,
                      "peak_how": f"{sm_count} SMs x 128 lanes x {sm_max:.0f} MHz (B300_MICROARCH.md: 1 warp-inst/clk/SMSP); DESIGN.md section 9"},
     }
+    if prune_flags:
+        # DESIGN.md 7.8/7.9: records identical to the exhaustive run, but plans are skipped, so `value` counts the
+        # (plan, level) evaluations COVERED, not executed: not the headline metric and no roofline claim.
+        line["config"]["pruning"] = f"{args.prune} (exact; value = evaluations covered, not executed; not the headline)"
+        line["bound_skipped_outer"] = int(st.get("bound_skipped", 0))
+        line["plans_enumerated_per_gpu"] = int(st["plans"])
+        line["roofline"]["frac"] = line["roofline"]["achieved"] = None
     if world == 1 and not args.no_cpu_baseline:
         sample = oracle_sample(w, args.cpu_requests)
         dt, ev, cores = time_oracle(sample)
@@ -432,6 +444,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--objective", default="product", choices=["product", "linear"],
                     help="product: north_star's constrained objective (default); linear: the paper's Eq.(4)/(5)")
+    ap.add_argument("--prune", default="none", choices=["none", "dominated", "bounds", "both"],
+                    help="opt-in exact pruning (DESIGN.md 7.8/7.9); the default, headline line never prunes")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "dyplan" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
