@@ -58,7 +58,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t pari
 }
 
 // ---- winner -> bundle record (S6), one thread per (request, level) ---------------------------------------------
-static __device__ __noinline__ void emit_record(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) {
+static __device__ __forceinline__ void emit_record(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) {
   const dyplan_batch& b = a.in;
   const dyplan_bundle& o = a.out;
   const int B = b.B, M = b.M;
