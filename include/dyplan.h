@@ -278,6 +278,22 @@ typedef struct {
 /* Synchronises `stream` of the last call, then fills *out. */
 DYPLAN_API int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out);
 
+/* M0: the measured issue rate of the instructions the scorers are made of, on
+ * THIS device -- the denominator of the path's roofline ("bound": "alu").  For each entry the library runs a kernel
+ * of independent dependency chains of that one SASS instruction (or of the scorer's own instruction mix), one block per
+ * SM with 8 warps per SMSP, and reports executed warp-instructions per clock per SMSP from clock64() stamps: the median
+ * over the SMs (rate), the slowest and fastest SM.  sm_clock_mhz (optional) receives the SM clock the kernels held
+ * (cycles of the longest block / CUDA-event time).  `out` is a HOST array of `capacity` entries; *n_out receives the
+ * number written (all of them if capacity allows; DYPLAN_ERR_ARG if capacity < 1).  Synchronises `stream`. */
+typedef struct {
+  char name[64];   /* SASS mnemonic, or "mix: ..." for an instruction mix                           */
+  float rate;      /* warp-instructions / clk / SMSP, median over the SMs (1.0 = the issue port)    */
+  float rate_min;  /* slowest SM                                                                    */
+  float rate_max;  /* fastest SM                                                                    */
+} dyplan_issue_rate;
+DYPLAN_API int dyplan_measure_issue_rates(dyplan_ctx* ctx, dyplan_issue_rate* out, int32_t capacity, int32_t* n_out,
+                               float* sm_clock_mhz, void* stream);
+
 DYPLAN_API const char* dyplan_strerror(int code);
 DYPLAN_API const char* dyplan_last_cuda_error(const dyplan_ctx* ctx); /* "" if none */
 DYPLAN_API int dyplan_version(void);                            /* major*10000 + minor*100 + patch */

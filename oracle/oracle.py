@@ -1,7 +1,7 @@
 """ctypes binding of oracle/dyplan_oracle.c (TEST INFRASTRUCTURE, not product).
 
 Builds ``oracle/_build/liborc.so`` with gcc on first use.  Everything here takes the numpy
-``Batch`` / ``Workload`` of ``paper_2607_02942_b200.workloads`` (the shared input generator) and
+``Batch`` / ``Workload`` of ``tests/support/workloads.py`` (the shared seeded input generator) and
 returns plain dicts of numpy arrays.  Arithmetic lives in the C file; this file only marshals.
 """
 from __future__ import annotations

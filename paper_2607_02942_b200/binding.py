@@ -28,7 +28,7 @@ NO_IDX = np.iinfo(np.uint64).max
 EXPORTS = (
     "dyplan_create", "dyplan_destroy", "dyplan_set_flags", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_compile_linear_host", "dyplan_bind",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
-    "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version",
+    "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version", "dyplan_measure_issue_rates",
 )
 
 
@@ -79,6 +79,10 @@ class CStats(C.Structure):
                 ("bound_skipped", C.c_uint64)]
 
 
+class CIssueRate(C.Structure):
+    _fields_ = [("name", C.c_char * 64), ("rate", C.c_float), ("rate_min", C.c_float), ("rate_max", C.c_float)]
+
+
 _lib = None
 
 
@@ -106,6 +110,7 @@ def lib():
         l.dyplan_replan_host.argtypes = [vp, pb, vp, vp, vp, u32, po, vp, pu64, pu64]
         l.dyplan_select_host.argtypes = [vp, pb, po, i32, vp, vp, po, vp, pu64, pu64]
         l.dyplan_last_stats.argtypes = [vp, C.POINTER(CStats)]
+        l.dyplan_measure_issue_rates.argtypes = [vp, C.POINTER(CIssueRate), i32, C.POINTER(i32), C.POINTER(C.c_float), vp]
         for n in EXPORTS:
             getattr(l, n).restype = C.c_int
         l.dyplan_strerror.restype = C.c_char_p
@@ -347,6 +352,14 @@ class Context:
                                              C.byref(rescored.cstruct) if rescored is not None else None,
                                              _stream_ptr(stream), C.byref(h2d), C.byref(d2h)))
         return h2d.value, d2h.value
+
+    def dyplan_measure_issue_rates(self, stream=None):
+        """M0: ([{name, rate, rate_min, rate_max}], sm_clock_mhz) -- warp-instructions / clk / SMSP per instruction."""
+        arr = (CIssueRate * 32)()
+        n, mhz = C.c_int32(), C.c_float()
+        self._check(lib().dyplan_measure_issue_rates(self._h, arr, 32, C.byref(n), C.byref(mhz), _stream_ptr(stream)))
+        return ([dict(name=arr[i].name.decode(), rate=arr[i].rate, rate_min=arr[i].rate_min, rate_max=arr[i].rate_max)
+                 for i in range(n.value)], mhz.value)
 
     def dyplan_last_stats(self) -> dict:
         st = CStats()

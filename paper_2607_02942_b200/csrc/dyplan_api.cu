@@ -377,6 +377,64 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   return DYPLAN_OK;
 }
 
+int dyplan_measure_issue_rates(dyplan_ctx* ctx, dyplan_issue_rate* out, int32_t capacity, int32_t* n_out, float* sm_clock_mhz,
+                               void* stream) {
+  if (!ctx || !out || !n_out) return DYPLAN_ERR_NULL;
+  if (capacity < 1) return DYPLAN_ERR_ARG;
+  *n_out = 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  const int grid = ctx->sm_count, wpb = m0_warps_per_block();
+  const size_t nst = (size_t)grid * wpb * 2;
+  int rc;
+  if ((rc = ensure(ctx, ctx->arena, nst * sizeof(long long) + 256))) return rc;
+  long long* d_st = (long long*)ctx->arena.p;
+  float* d_sink = (float*)((char*)ctx->arena.p + nst * sizeof(long long));
+  long long* h_st = new (std::nothrow) long long[nst];
+  float* rates = new (std::nothrow) float[grid];
+  if (!h_st || !rates) { delete[] h_st; delete[] rates; return DYPLAN_ERR_ARG; }
+  const int n = m0_count() < capacity ? m0_count() : capacity;
+  double clk_sum = 0.0;
+  int clk_n = 0;
+  cudaError_t e = cudaSuccess;
+  for (int op = 0; op < n && e == cudaSuccess; op++) {
+    if ((e = m0_launch(op, grid, d_st, d_sink, s)) != cudaSuccess) break;   // warm-up (instruction cache, clocks)
+    if ((e = cudaEventRecord(ctx->ev0, s)) != cudaSuccess) break;
+    if ((e = m0_launch(op, grid, d_st, d_sink, s)) != cudaSuccess) break;
+    if ((e = cudaEventRecord(ctx->ev1, s)) != cudaSuccess) break;
+    if ((e = cudaMemcpyAsync(h_st, d_st, nst * sizeof(long long), cudaMemcpyDeviceToHost, s)) != cudaSuccess) break;
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) break;
+    float ms = 0.f;
+    if ((e = cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1)) != cudaSuccess) break;
+    long long longest = 0;
+    for (int b = 0; b < grid; b++) {
+      long long t0 = h_st[(size_t)b * wpb * 2], t1 = h_st[(size_t)b * wpb * 2 + 1];
+      for (int w = 1; w < wpb; w++) {
+        const long long a0 = h_st[((size_t)b * wpb + w) * 2], a1 = h_st[((size_t)b * wpb + w) * 2 + 1];
+        t0 = a0 < t0 ? a0 : t0; t1 = a1 > t1 ? a1 : t1;
+      }
+      const long long cyc = t1 - t0 > 0 ? t1 - t0 : 1;
+      longest = cyc > longest ? cyc : longest;
+      rates[b] = (float)((double)wpb * m0_warp_inst_per_warp() / 4.0 / (double)cyc);
+    }
+    for (int i = 1; i < grid; i++) {   // insertion sort: grid = 148
+      const float v = rates[i]; int j = i - 1;
+      while (j >= 0 && rates[j] > v) { rates[j + 1] = rates[j]; j--; }
+      rates[j + 1] = v;
+    }
+    memset(out[op].name, 0, sizeof(out[op].name));
+    strncpy(out[op].name, m0_name(op), sizeof(out[op].name) - 1);
+    out[op].rate = rates[grid / 2]; out[op].rate_min = rates[0]; out[op].rate_max = rates[grid - 1];
+    if (ms > 0.f) { clk_sum += (double)longest / ((double)ms * 1e3); clk_n++; }   // cycles per microsecond = MHz
+  }
+  delete[] h_st; delete[] rates;
+  if (e != cudaSuccess) return fail_cuda(ctx, e);
+  *n_out = n;
+  if (sm_clock_mhz) *sm_clock_mhz = clk_n ? (float)(clk_sum / clk_n) : 0.f;
+  ctx->last_launches = 2 * n; ctx->have_events = false; ctx->last_stream = s;
+  return DYPLAN_OK;
+}
+
 int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
   if (!ctx || !out) return DYPLAN_ERR_NULL;
   memset(out, 0, sizeof(*out));

@@ -543,12 +543,16 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
       Partial p; p.C = mine.C; p.T = mine.T; p.idx = mine.idx;
       a.partial[(size_t)(rec_base + item) * Lr + lane] = p;
       if (mine.idx != kNoIdx) atomicMax(&g_thr[lane], __float_as_int(mine.C));
-      __threadfence();
     }
     __syncwarp();
     const uint32_t n_it = __ldg(&a.item_off_f[r + 1]) - first_item;
     uint32_t last = 0;
-    if (lane == 0) last = (atomicAdd(&a.done[r], 1u) == n_it - 1) ? 1u : 0u;
+    if (lane == 0) {
+      // release: the lanes' record stores happen-before lane 0's fence (warp barrier), the fence is cumulative at gpu
+      // scope and precedes the ticket in the same thread -- the pattern the PTX memory model orders
+      __threadfence();
+      last = (atomicAdd(&a.done[r], 1u) == n_it - 1) ? 1u : 0u;
+    }
     last = __shfl_sync(0xffffffffu, last, 0);
     if (last) {
       // ---- last warp of this request: reduce its items' records and emit the bundle (fused K_final) ----

@@ -190,6 +190,13 @@ struct LinArgs {
 };
 cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s);
 
+// ---- M0 issue-rate micro-benchmarks (dyplan_m0.cu) ----
+int m0_count();
+const char* m0_name(int op);
+int m0_warps_per_block();
+double m0_warp_inst_per_warp();
+cudaError_t m0_launch(int op, int grid, long long* stamps, float* sink, cudaStream_t s);
+
 __host__ __device__ inline int nb_class_of(int B, bool has_caps) { return !has_caps ? 0 : (B <= 2 ? 2 : (B <= 4 ? 4 : 8)); }
 
 }  // namespace dyplan

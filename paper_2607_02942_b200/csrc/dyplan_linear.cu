@@ -236,7 +236,12 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
       unsigned long long kk = best[l] == v ? kmin[l] : ~0ull;
 #pragma unroll
       for (int off = 16; off; off >>= 1) { const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, kk, off); kk = o2 < kk ? o2 : kk; }
-      if (lane == 0) { LinRec rc; rc.J = v; rc.pad = 0; rc.key = kk; a.rec[((size_t)r * a.chunks + c) * L + l] = rc; }
+      if (lane == 0) {
+        LinRec rc; rc.J = v; rc.pad = 0; rc.key = kk; a.rec[((size_t)r * a.chunks + c) * L + l] = rc;
+        // publish: later items of this request start from a J that one of its plans attains (ties still pass the
+        // dj >= 0 test and the key decides, so the result does not depend on what is published when)
+        if (kk != ~0ull) atomicMax(&a.gJ[r * L + l], enc_f32(v));
+      }
     }
   }
 }

@@ -348,11 +348,11 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) k_score(const CallArgs a) 
       Partial p; p.C = v.C; p.T = v.T; p.idx = v.idx;
       a.partial[(size_t)item * L + tid] = p;
       if (v.idx != kNoIdx) atomicMax(&g_thr[tid], __float_as_int(v.C));
-      __threadfence();
     }
     __syncthreads();
     if (tid == 0) {
       const uint32_t n_it = a.item_off[r + 1] - first_item;
+      __threadfence();   // release in the ticket-taking thread, after the block barrier (cumulative over the records above)
       const uint32_t t = atomicAdd(&a.done[r], 1u);
       s_last = (t == n_it - 1) ? 1u : 0u;
     }

@@ -31,9 +31,15 @@ __device__ __forceinline__ int nth_set_bit(uint32_t m, int k) {
 
 // Exact per-node dominance pruning: option x of a node can be dropped when another
 // option y of the same node is at least as good in every quantity the objective reads -- factor f (as the scorer's
-// fp32 value), every level's scaled duration, and with caps the same backend and no more demand -- and is strictly
-// preferred by order 7 (f larger, or f equal and a lower option index).  Swapping x for y in any plan keeps it feasible
-// (durations enter T monotonically) and makes it strictly better, so no dropped option is in any best plan.
+// fp32 value), every level's scaled duration, and with caps the same backend and no more demand -- and the plan with y
+// in place of x is STRICTLY preferred by the order the scorer applies: (C32 desc, T asc, idx asc), C32 being the fp32
+// product in the scorer's fixed node order.  Rounding is monotone, so fy >= fx gives C32(y-plan) >= C32(x-plan) and
+// T(y-plan) <= T(x-plan); that is strict when y < x (lower canonical index breaks the last tie).  For y > x the index
+// speaks for x, so C32 itself must separate: the exact products differ by the factor fy / fx, each fp32 product of
+// <= 16 factors is within 16 * 2^-24 of exact, hence fy >= fx (1 + 2^-18) (3.8e-6 > 2 * 0.96e-6) keeps
+// C32(y-plan) > C32(x-plan).  (Factors a few ulps apart -- tiny v -- round to equal products; x then wins the tie-break
+// of the full enumeration and must be kept.)  The relation is transitive and acyclic: every dropped option is
+// dominated by a kept one, and no dropped option is in any best plan.
 __device__ uint32_t dominance_keep(const dyplan_batch& b, int o0, int K, float v, const int* mult, int L, int B, bool has_caps) {
   uint32_t keep = K >= 32 ? 0xffffffffu : ((1u << K) - 1u);
   for (int x = 0; x < K; x++) {
@@ -44,7 +50,8 @@ __device__ uint32_t dominance_keep(const dyplan_batch& b, int o0, int K, float v
       const int oy = o0 + y;
       if (has_caps && (b.backend[oy] != b.backend[ox] || b.demand[oy] > b.demand[ox])) continue;
       const float fy = (float)factor64(v, b.acc[oy]);
-      if (!(fy > fx || (fy == fx && y < x))) continue;
+      const bool separated = (double)fy >= __dmul_rn((double)fx, 1.0 + 1.0 / 262144.0) && fy > fx;
+      if (!(separated || (fy >= fx && y < x))) continue;
       bool ok = true;
       for (int l = 0; l < L && ok; l++)
         ok = scaled(b.lat_us[oy], mult[l * B + b.backend[oy]]) <= scaled(b.lat_us[ox], mult[l * B + b.backend[ox]]);

@@ -1,7 +1,7 @@
 """Seeded synthetic inputs for the dyplan hot path (numpy only).
 
-This module is the ONE thing the oracle-side tests and the CUDA-side binding /
-bench share.  It produces flat little-endian arrays in exactly the layout of
+This module is the ONE thing the oracle-side tests and the CUDA-side tests /
+bench / smoke share (test support: it is not part of the shipped package).  It produces flat little-endian arrays in exactly the layout of
 ``include/dyplan.h`` (``dyplan_batch``) and nothing else: it contains no
 enumeration, no arg-best, no correctness product and no demand accounting --
 i.e. none of the method's arithmetic.  The one piece of workload *recipe* that
@@ -447,10 +447,23 @@ def random_workload(seed: int, R: int, nmin: int, nmax: int, kmin: int, kmax: in
                     mult_pm=np.ascontiguousarray(mult.reshape(-1)), meta=dict(seed=seed))
 
 
+def random_down_set(rng, pred_masks, p: float) -> int:
+    """A random predecessor-closed node set (a down-set of the DAG): visit the nodes in topological order and take
+    a node with probability ``p`` if all its predecessors were taken.  PAPER.md:129: a node is dispatched only after
+    its predecessors finished; PAPER.md:521-530 (App. D): the committed bindings are a set, not a prefix."""
+    m = 0
+    for v, pm in enumerate(pred_masks):
+        if (int(pm) & ~m) == 0 and rng.random() < p:
+            m |= 1 << v
+    return m
+
+
 def random_replan_workload(seed: int, R: int, nmin: int, nmax: int, kmin: int, kmax: int, B: int = 2, M: int = 3,
-                           *, caps: bool = True, flags: int = FLAG_FIXED_IN_PLACE, tool_p: float = 0.1) -> Workload:
-    """Replan queries with a predecessor-closed dispatched set: a random prefix of the node
-    order (any prefix of a topological order is predecessor-closed)."""
+                           *, caps: bool = True, flags: int = FLAG_FIXED_IN_PLACE, tool_p: float = 0.1,
+                           shape: str = "mixed") -> Workload:
+    """Replan queries with a predecessor-closed dispatched set.  ``shape``: "prefix" = a random prefix of the node
+    order (any prefix of a topological order is predecessor-closed); "downset" = a random down-set of the DAG, in
+    general NOT a prefix (nodes {0, 2} when 2 does not depend on 1); "mixed" = either, per query."""
     w = random_workload(seed, R, nmin, nmax, kmin, kmax, B, M, L=1, caps=caps, tool_p=tool_p)
     rng = np.random.default_rng(seed + 7919)
     b = w.batch
@@ -463,7 +476,41 @@ def random_replan_workload(seed: int, R: int, nmin: int, nmax: int, kmin: int, k
         rad = b.radices(r)
         for i in range(n):
             fc[b.node_off[r] + i] = int(rng.integers(0, rad[i]))
+    if shape != "prefix":
+        rng2 = np.random.default_rng(seed + 104729)
+        for r in range(R):
+            if shape == "mixed" and rng2.random() < 0.35:
+                continue
+            pm = b.pred_mask[b.node_off[r]: b.node_off[r + 1]]
+            disp[r] = random_down_set(rng2, pm, float(rng2.uniform(0.3, 0.9)))
     live = rng.integers(1000, 4001, size=(R, B)).astype(np.int32)
-    return Workload(name=f"random_replan(seed={seed},R={R})", kind="replan", batch=b, L=1,
+    return Workload(name=f"random_replan(seed={seed},R={R},{shape})", kind="replan", batch=b, L=1,
                     dispatched_mask=disp, fixed_choice=fc, live_mult_pm=np.ascontiguousarray(live.reshape(-1)),
                     flags=flags, meta=dict(seed=seed))
+
+
+def with_down_set_dispatch(w: Workload, seed: int, p_lo: float = 0.3, p_hi: float = 0.8, max_free_plans: int = 1 << 26,
+                           flags: Optional[int] = None) -> Workload:
+    """The replan workload ``w`` (e.g. configs[3]) with every query's dispatched set redrawn as a random down-set of
+    its DAG (not a prefix) and a uniformly drawn fixed option on every node; all other inputs unchanged.  A draw that
+    leaves more than ``max_free_plans`` plans to enumerate is redrawn (keeps the oracle affordable)."""
+    assert w.kind == "replan"
+    rng = np.random.default_rng(seed)
+    b = w.batch
+    disp = np.zeros(b.R, dtype=np.uint32)
+    fc = np.zeros(b.NN, dtype=np.uint8)
+    for r in range(b.R):
+        n0, n1 = int(b.node_off[r]), int(b.node_off[r + 1])
+        rad = b.radices(r)
+        fc[n0:n1] = [int(rng.integers(0, k)) for k in rad]
+        for _ in range(64):
+            m = random_down_set(rng, b.pred_mask[n0:n1], float(rng.uniform(p_lo, p_hi)))
+            free = 1
+            for i, k in enumerate(rad):
+                if not (m >> i) & 1:
+                    free *= int(k)
+            if free <= max_free_plans:
+                break
+        disp[r] = m
+    return replace(w, name=w.name + "+downsets", dispatched_mask=disp, fixed_choice=fc,
+                   flags=w.flags if flags is None else flags)

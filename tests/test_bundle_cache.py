@@ -4,7 +4,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 from paper_2607_02942_b200.cache import BundleCache, request_key
 
 FIELDS = ("plan_idx", "choice", "corr", "lat", "dem", "dom_model", "status")

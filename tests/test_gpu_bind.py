@@ -5,7 +5,7 @@ from __future__ import annotations
 import numpy as np
 import pytest
 
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 
 pytestmark = pytest.mark.gpu
 

@@ -8,7 +8,7 @@ from __future__ import annotations
 import numpy as np
 import pytest
 
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 
 from parity import check_records
 
@@ -122,6 +122,30 @@ def test_random_replan(dy, orc, seed, flags):
     nd = np.array([bin(int(m)).count("1") for m in w.dispatched_mask])
     nn = np.array([w.batch.n_nodes(r) for r in range(w.batch.R)])
     assert (nd == nn).any() and (nd == 0).any()
+
+
+@pytest.mark.parametrize("seed,flags", [(35, wl.FLAG_FIXED_IN_PLACE), (36, wl.FLAG_RESIDUAL), (37, wl.FLAG_FIXED_IN_PLACE)])
+def test_random_replan_non_prefix_down_sets(dy, orc, seed, flags):
+    """Dispatched sets that are predecessor-closed but NOT a prefix of the node order (nodes {0, 2} when 2 does not
+    depend on 1): valid under include/dyplan.h and App. D; k_stage's orientation, pinned node 0
+    and base_idx paths differ from the prefix case."""
+    w = wl.random_replan_workload(seed, R=64, nmin=3, nmax=9, kmin=1, kmax=5, B=3, M=3, caps=(seed != 37), flags=flags,
+                                  shape="downset")
+    m = w.dispatched_mask.astype(np.int64)
+    assert ((m & (m + 1)) != 0).sum() >= 16, "too few non-prefix sets drawn"
+    # node 0 free while later nodes are pinned, and the last node pinned while earlier ones are free
+    nn = np.array([w.batch.n_nodes(r) for r in range(w.batch.R)])
+    assert (((m & 1) == 0) & (m != 0)).any() and (((m >> (nn - 1)) & 1 == 1) & (m != (1 << nn) - 1)).any()
+    both(dy, orc, w, f"replan-downsets(seed={seed})")
+
+
+def test_cfg3_shape_non_prefix_down_sets_both_flags(dy, orc):
+    base = wl.make_config(3, R=160)
+    for flags in (wl.FLAG_FIXED_IN_PLACE, wl.FLAG_RESIDUAL):
+        w = wl.with_down_set_dispatch(base, seed=77, max_free_plans=12 ** 5, flags=flags)
+        m = w.dispatched_mask.astype(np.int64)
+        assert ((m & (m + 1)) != 0).sum() >= 60
+        both(dy, orc, w, f"cfg3-downsets(flags={flags})")
 
 
 def test_slo_sweep_monotone_and_infeasible(dy, orc):
@@ -576,3 +600,61 @@ def test_bounds_and_dominance_pruning_together(dy, orc):
         assert e.value.code == binding.ERR_ARG
     finally:
         ctx.dyplan_set_flags(0)
+
+
+# ---- both prunings: records identical BIT FOR BIT to the exhaustive GPU run (not only to the oracle within 1e-5) -----
+def _near_tie_workload(seed, R=24, L=2, B=2, caps=False):
+    """Tie-heavy inputs for the pruning A/B test: vulnerabilities around 1e-7 (every factor 1 - v(1 - a) lands within
+    a few fp32 ulps of 1, so products of distinct factors round to equal C32) and few distinct durations (T ties),
+    so the canonical-index tie-break decides most records."""
+    rng = np.random.default_rng(seed)
+    w = wl.random_workload(seed, R=R, nmin=2, nmax=6, kmin=2, kmax=8, B=B, M=3, L=L, caps=caps, tool_p=0.0)
+    b = w.batch
+    b.vuln[:] = rng.choice([0.0, 5e-8, 1e-7, 2e-7, 1e-6], size=b.vuln.size).astype(np.float32)
+    half = rng.random(b.R) < 0.5
+    for r in range(b.R):
+        n0, n1 = int(b.node_off[r]), int(b.node_off[r + 1])
+        o0, o1 = int(b.opt_off[n0]), int(b.opt_off[n1])
+        if half[r]:
+            b.lat_us[o0:o1] = 500                                   # all durations equal: T ties everywhere
+        else:
+            b.lat_us[o0:o1] = rng.choice([400, 500], size=o1 - o0)
+        b.slo_us[r] = 500 * (n1 - n0) * 4
+    return w
+
+
+def _gpu_with_flags(dy, w, flags):
+    binding, ctx = dy
+    ctx.dyplan_set_flags(flags)
+    try:
+        g = gpu_run(dy, w)
+        st = ctx.dyplan_last_stats()
+    finally:
+        ctx.dyplan_set_flags(0)
+    return g, st
+
+
+@pytest.mark.parametrize("seed,L,B,caps", [(141, 1, 1, False), (142, 2, 2, False), (143, 3, 2, True), (144, 4, 3, True)])
+def test_prunings_are_bit_identical_to_the_exhaustive_run_on_near_ties(dy, orc, seed, L, B, caps):
+    binding, _ = dy
+    w = _near_tie_workload(seed, L=L, B=B, caps=caps)
+    base, st0 = _gpu_with_flags(dy, w, 0)
+    check_records(orc, w, base, orc.run(w), where=f"near-ties(seed={seed})")
+    for flags in (binding.PRUNE_DOMINATED, binding.PRUNE_BOUNDS, binding.PRUNE_DOMINATED | binding.PRUNE_BOUNDS):
+        g, st = _gpu_with_flags(dy, w, flags)
+        for k in ("status", "plan_idx", "choice", "corr", "corr64", "lat", "dem", "dom_model"):
+            assert np.array_equal(base[k], g[k]), f"flags={flags}: {k} differs from the exhaustive run"
+
+
+@pytest.mark.parametrize("seed", [151, 152])
+def test_prunings_are_bit_identical_on_ordinary_batches(dy, orc, seed):
+    binding, _ = dy
+    ws = [wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=8, B=3, M=3, L=4, caps=True),
+          wl.make_config(2, R=16), wl.make_config(1, R=2)]
+    ws.append(wl.random_replan_workload(seed, R=40, nmin=1, nmax=8, kmin=1, kmax=6, B=3, M=3, caps=True))
+    for w in ws:
+        base, _ = _gpu_with_flags(dy, w, 0)
+        for flags in (binding.PRUNE_DOMINATED, binding.PRUNE_BOUNDS, binding.PRUNE_DOMINATED | binding.PRUNE_BOUNDS):
+            g, _ = _gpu_with_flags(dy, w, flags)
+            for k in ("status", "plan_idx", "choice", "corr", "corr64", "lat", "dem", "dom_model"):
+                assert np.array_equal(base[k], g[k]), f"{w.name} flags={flags}: {k} differs from the exhaustive run"

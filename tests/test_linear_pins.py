@@ -13,7 +13,7 @@ import pytest
 
 from conftest import read_golden
 from oracle import linear as lo
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 
 P0 = dict(lambda_f=0.5, lambda_c=0.1, lambda_l=0.0005, lambda_ld=0.0002, beta=0.5, effort=1.0)
 

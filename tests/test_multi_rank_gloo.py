@@ -13,7 +13,7 @@ import numpy as np
 import pytest
 
 from paper_2607_02942_b200 import multi
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 
 
 def test_shard_requests_is_a_balanced_partition():

@@ -13,7 +13,7 @@ import numpy as np
 import pytest
 
 from conftest import read_golden
-from paper_2607_02942_b200 import workloads as wl
+from support import workloads as wl
 
 U64MAX = np.iinfo(np.uint64).max
 
@@ -421,26 +421,32 @@ def test_diamond_cfg0_shape_vs_recursive_solver(orc):
 
 
 # ---------------------------------------------------------------- PIN12 replan consistency
-def test_pin12_replan_consistency(orc):
-    w = wl.random_replan_workload(12, R=30, nmin=2, nmax=5, kmin=2, kmax=4, caps=True)
+# The dispatched set is any predecessor-closed node set (dispatch needs finished predecessors;
+# PAPER.md:521-530 App. D: the committed bindings are a set), so each pin runs on prefixes and on general down-sets.
+@pytest.mark.parametrize("shape", ["prefix", "downset"])
+def test_pin12_replan_consistency(orc, shape):
+    w = wl.random_replan_workload(12, R=30, nmin=2, nmax=5, kmin=2, kmax=4, caps=True, shape=shape)
     b = w.batch
     live = w.live_mult_pm.reshape(b.R, b.B)
     out = orc.replan(b, w.dispatched_mask, w.fixed_choice, w.live_mult_pm, wl.FLAG_FIXED_IN_PLACE)
+    non_prefix = 0
     for r in range(b.R):
         n = b.n_nodes(r)
-        d = int(w.dispatched_mask[r]).bit_count()
-        fixed = {i: int(w.fixed_choice[b.node_off[r] + i]) for i in range(d)}
-        # fixed prefix == compile's enumeration filtered to plans agreeing with the prefix (independent solver)
+        m = int(w.dispatched_mask[r])
+        non_prefix += (m & (m + 1)) != 0
+        fixed = {i: int(w.fixed_choice[b.node_off[r] + i]) for i in range(n) if (m >> i) & 1}
+        # fixed set == compile's enumeration filtered to plans agreeing with the fixed bindings (independent solver)
         _check_against_rec(out, r, RecSolver(b, r, live[r], fixed=fixed).solve())
         if out["status"][r] == 0:
-            for i in range(d):   # "the merge rejects overlap instead of replacing a committed binding" PAPER.md:528
+            for i in fixed:      # "the merge rejects overlap instead of replacing a committed binding" PAPER.md:528
                 assert int(out["choice"][r][i]) == fixed[i]
-        if d == n:               # "If U_t is empty, there are no remaining choices" PAPER.md:528
+        if len(fixed) == n:      # "If U_t is empty, there are no remaining choices" PAPER.md:528
             s = orc.score(b, r, live[r], [fixed[i] for i in range(n)])
             assert (out["status"][r] == 0) == s["feasible"]
             if s["feasible"]:
                 assert int(out["plan_idx"][r]) == s["plan_idx"] and out["corr"][r] == s["corr"]
                 assert int(out["lat"][r]) == s["lat"] and int(out["n_feasible"][r]) == 1
+    assert (non_prefix >= 5) == (shape == "downset")
     # no node dispatched == compile at that single level
     zero = np.zeros(b.R, np.uint32)
     o0 = orc.replan(b, zero, w.fixed_choice, w.live_mult_pm, 0)
@@ -450,22 +456,25 @@ def test_pin12_replan_consistency(orc):
             assert o0[key][r] == oc[key][0], key
 
 
-def test_pin12_residual_equals_compile_on_induced_subdag(orc):
-    w = wl.random_replan_workload(13, R=25, nmin=2, nmax=5, kmin=2, kmax=4, caps=True, flags=wl.FLAG_RESIDUAL)
+@pytest.mark.parametrize("shape", ["prefix", "downset"])
+def test_pin12_residual_equals_compile_on_induced_subdag(orc, shape):
+    w = wl.random_replan_workload(13, R=25, nmin=2, nmax=5, kmin=2, kmax=4, caps=True, flags=wl.FLAG_RESIDUAL, shape=shape)
     b = w.batch
     live = w.live_mult_pm.reshape(b.R, b.B)
     out = orc.replan(b, w.dispatched_mask, w.fixed_choice, w.live_mult_pm, wl.FLAG_RESIDUAL)
     for r in range(b.R):
         n = b.n_nodes(r)
-        d = int(w.dispatched_mask[r]).bit_count()
+        m = int(w.dispatched_mask[r])
         n0 = int(b.node_off[r])
-        # G[U_t]: drop the first d nodes, shift predecessor bits
-        sub = dict(pred_mask=[int(b.pred_mask[n0 + v]) >> d for v in range(d, n)],
-                   vuln=[float(b.vuln[n0 + v]) for v in range(d, n)], slo=int(b.slo_us[r]),
+        U = [v for v in range(n) if not (m >> v) & 1]      # undispatched nodes, in order
+        # G[U_t]: the sub-DAG induced by the undispatched nodes; predecessor bits renumbered
+        pos = {v: i for i, v in enumerate(U)}
+        sub = dict(pred_mask=[sum(1 << pos[u] for u in U if (int(b.pred_mask[n0 + v]) >> u) & 1) for v in U],
+                   vuln=[float(b.vuln[n0 + v]) for v in U], slo=int(b.slo_us[r]),
                    cap=[int(x) for x in b.cap[r * b.B:(r + 1) * b.B]])
         for key, arr in (("lat", b.lat_us), ("acc", b.acc), ("demand", b.demand), ("backend", b.backend), ("model", b.model)):
-            sub[key] = [[arr[o].item() for o in range(b.opt_off[n0 + v], b.opt_off[n0 + v + 1])] for v in range(d, n)]
-        if d == n:
+            sub[key] = [[arr[o].item() for o in range(b.opt_off[n0 + v], b.opt_off[n0 + v + 1])] for v in U]
+        if not U:
             assert out["status"][r] == 0 and out["corr"][r] == 1.0 and out["lat"][r] == 0
             continue
         oc = orc.compile(mk([sub], b.B, b.M, True), 1, live[r])
@@ -474,7 +483,7 @@ def test_pin12_residual_equals_compile_on_induced_subdag(orc):
         if oc["status"][0] == 0:
             assert out["corr"][r] == oc["corr"][0] and int(out["lat"][r]) == int(oc["lat"][0])
             assert (out["dem"][r] == oc["dem"][0]).all()
-            assert [int(x) for x in out["choice"][r][d:n]] == [int(x) for x in oc["choice"][0][: n - d]]
+            assert [int(out["choice"][r][v]) for v in U] == [int(x) for x in oc["choice"][0][: len(U)]]
 
 
 def test_replan_rejects_non_predecessor_closed_dispatch(orc):
