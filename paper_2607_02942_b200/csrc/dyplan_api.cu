@@ -213,7 +213,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   // persistent grids: every block resident, work pulled from device counters
   const int grid = ctx->sm_count * occ;
   const int fgrid = ctx->sm_count * focc;
-  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * 16u;
+  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * kFastItemsPerWarp;
   const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * (target_items_f > 32768u ? target_items_f : 32768u);
   if ((rc = ensure(ctx, ctx->blob, R * blob_stride_words(L) * 4))) return rc;
   if ((rc = ensure(ctx, ctx->item_off, 2 * (R + 1) * 4))) return rc;

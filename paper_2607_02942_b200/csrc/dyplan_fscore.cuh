@@ -255,10 +255,18 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     const bool live = step < my_count;
     const int slot2 = ob2 + k2;
     float R2[L], U1pS[L], A0q1[L];
+    float4 c4v[L];
+    if (kCtxShared) {
+      // all L loads are issued back to back (program-ordered asm), so their latencies overlap instead of chaining
+      // through one reused register quad
+#pragma unroll
+      for (int l = 0; l < L; l++)
+        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(c4v[l].x), "=f"(c4v[l].y), "=f"(c4v[l].z), "=f"(c4v[l].w) : "r"(smem_u32(cx + l * 32)));
+    }
 #pragma unroll
     for (int l = 0; l < L; l++) {
       float4 c4;
-      if (kCtxShared) c4 = cx[l * 32]; else c4 = make_float4(X2r[l], Rm3r[l], U1rr[l], A0rr[l]);
+      if (kCtxShared) c4 = c4v[l]; else c4 = make_float4(X2r[l], Rm3r[l], U1rr[l], A0rr[l]);
       const float u2 = c4.x + s_nlat[slot2 * L + l];
       R2[l] = fminf(c4.y, u2);
       const float U1 = fminf(c4.z, u2 + big12);
@@ -276,20 +284,25 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     }
 
     float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
+    // node 1's options are walked by pointer (factor, [L] durations, [8] per-backend demands): an index loop cost four
+    // more ALU-pipe instructions per pair of groups for the address arithmetic (measured: 4.6 % of cfg1's time)
+    const float* pf1 = s_f + K0P;
+    const float* const pf1_end = pf1 + K1;
+    const float* pn1 = s_nlat + K0P * L;
+    const float* pd1 = s_dem1b;
 #pragma unroll 2
-    for (int k1 = 0; k1 < K1; k1++) {
-      const int slot1 = K0P + k1;
-      float C1 = C2 * s_f[slot1];
+    for (; pf1 != pf1_end; pf1++, pn1 += L, pd1 += 8) {
+      float C1 = C2 * pf1[0];
       float s1[NBX];
       if (NB) {
         float smin = kBigF;
 #pragma unroll
-        for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - s_dem1b[k1 * 8 + b]; smin = fminf(smin, s1[b]); }
+        for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - pd1[b]; smin = fminf(smin, s1[b]); }
         C1 *= __saturatef(smin);   // a backend is already over its cap: no plan of this group can be a candidate
       }
       float ap1[L];
 #pragma unroll
-      for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(s_nlat[slot1 * L + l], S01, U1pS[l]));
+      for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(pn1[l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
       float zodd = 0.0f;             // odd L: the last level of an even k0 waits for the one of k0 + 1 (one FMNMX3 for both)
       float addend[L];
@@ -448,6 +461,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
   const uint32_t rec_base = a.st->total_items;          // partial records of the wide class come first
   const unsigned long long pif = a.st->per_item_outer_f;
   const bool small_call = a.st->small_call_f != 0;
+  const uint32_t tail_start = a.st->tail_start_f;
   if (lane == 0) mbar_init(&ws->bar, 1);
   __syncwarp();
   uint32_t phase = 0;
@@ -483,7 +497,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (lane < 8) { Best e; e.C = -1.0f; e.T = INT32_MAX; e.idx = kNoIdx; ws->best[lane] = e; }
     __syncwarp();
     const uint32_t first_item = __ldg(&a.item_off_f[r]);
-    const unsigned long long pir = fast_item_outer(pif, h->Kp[2], small_call);
+    const unsigned long long pir = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_call);
     const unsigned long long ob = (unsigned long long)(item - first_item) * pir;
     const unsigned long long oe = min(ob + pir, (unsigned long long)h->outer_total);
     const unsigned long long len = oe - ob;

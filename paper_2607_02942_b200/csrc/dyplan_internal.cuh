@@ -22,6 +22,7 @@ constexpr int kClassWide = 0;        // int32 slack DP (k_score): any request th
 constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): every latency / demand sum below 2^22, tables <= kFastBlobWords
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
+constexpr uint32_t kFastItemsPerWarp = 12;   // work items to aim for per resident warp (measured: 8 and 24 lose 4-7 % on cfg4)
 constexpr float kBigF = 16777216.0f; // 2^24
 // fast class: outer indices per work item of a request whose node 2 has K2 options -- the call-wide figure rounded up
 // so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)
@@ -88,7 +89,13 @@ struct CallState {
   uint32_t next_item_f;
   uint32_t fast_requests;           // requests staged for the fp32 scorer
   uint32_t small_call_f;            // fast class: fewer than ~1K outer indices per resident warp (items are not lane-aligned)
+  uint32_t tail_start_f;            // fast class: requests >= this index are cut into 4x smaller items (they are handed out last: a short tail)
+  uint32_t pad0;
 };
+// outer indices per item of request r before rounding (k_plan and k_fscore must agree)
+__host__ __device__ inline unsigned long long fast_pif_of(unsigned long long pif, uint32_t tail_start, long long r) {
+  return (unsigned long long)r >= tail_start ? (pif / 4 < 32 ? 32 : pif / 4) : pif;
+}
 
 struct CallArgs {                   // passed by value to the kernels
   dyplan_batch in;
