@@ -336,7 +336,7 @@ def bench_one(args, ctx, binding, torch, dist, dev, rank, world, cfg, wide, peak
         entry = {
             "workload": workload_label(cfg, wide), "cfg": cfg, "wide": wide, "name": w.name, "kind": w.kind,
             "requests_per_gpu": int(w.batch.R), "plans_per_gpu": int(plans), "levels": int(w.L),
-            "fast_requests": int(st.get("fast_requests", 0)),
+            "fast_requests": int(st.get("fast_requests", 0)), "approx_requests": int(st.get("approx_requests", 0)),
             "value": whole_job_rate(evals, world, args.steps, tot_ms) / 1e9, "unit": UNIT,
             "ms_per_step": tot_ms / args.steps, "kernel_ms": k_ms / args.steps,
             "plans_per_s": world * plans * args.steps / (tot_ms * 1e-3),

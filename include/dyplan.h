@@ -274,6 +274,8 @@ typedef struct {
   int32_t sm_count;     /* SMs of the device                                                                      */
   float score_ms;       /* device time of the scoring kernel of the last call (CUDA events on `stream`)           */
   uint64_t bound_skipped; /* outer indices (assignments of all but the two innermost digits) skipped by DYPLAN_PRUNE_BOUNDS */
+  uint64_t approx_requests; /* of fast_requests: those whose latency or demand sums exceed 2^22, scored by the fp32 kernel as a
+                               conservative screen with every candidate verified in int32 (results identical)          */
 } dyplan_stats;
 /* Synchronises `stream` of the last call, then fills *out. */
 DYPLAN_API int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out);

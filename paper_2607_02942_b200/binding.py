@@ -76,7 +76,7 @@ class CProfiles(C.Structure):
 class CStats(C.Structure):
     _fields_ = [("plans", C.c_uint64), ("evals", C.c_uint64), ("work_items", C.c_uint64), ("slow_steps", C.c_uint64),
                 ("fast_requests", C.c_uint64), ("launches", C.c_int32), ("sm_count", C.c_int32), ("score_ms", C.c_float),
-                ("bound_skipped", C.c_uint64)]
+                ("bound_skipped", C.c_uint64), ("approx_requests", C.c_uint64)]
 
 
 class CIssueRate(C.Structure):

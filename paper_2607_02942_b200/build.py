@@ -21,6 +21,13 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
          "-Xcompiler", "-fvisibility=hidden"]
 
 
+# Per-source additions.  The fp32 scorer's enumeration loop is sensitive to ptxas' register assignment (operand bank
+# conflicts show up as dispatch stalls): the same loop measured 2.59 or 2.73 ms on configs[1] depending on unrelated
+# code elsewhere in the function.  Capping the L <= 4 instantiations at 126 registers gave the good assignment on every
+# config measured; the cap does not spill.
+EXTRA = {f"dyplan_fscore_l{l}.cu": ["-maxrregcount=126"] for l in (1, 2, 3, 4)}
+
+
 def sources() -> list[str]:
     return sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
 
@@ -36,7 +43,7 @@ def _compile(src: str, force: bool, hdr_mtime: float) -> str:
     spath = os.path.join(CSRC, src)
     if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(spath), hdr_mtime):
         return obj
-    cmd = [NVCC, *FLAGS, "-c", "-o", obj, spath]
+    cmd = [NVCC, *FLAGS, *EXTRA.get(src, []), "-c", "-o", obj, spath]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")

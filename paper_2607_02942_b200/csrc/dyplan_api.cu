@@ -459,6 +459,7 @@ int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
     out->fast_requests = st.fast_requests;
     out->slow_steps = st.slow_steps;
     out->bound_skipped = st.bound_skipped;
+    out->approx_requests = st.approx_requests;
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     out->score_ms = ms;

@@ -26,12 +26,12 @@ struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
   Best best[8];                    // the warp's incumbent per level (written by the cooperative slow path only)
   int thr[8];                      // bits of the best C seen so far per level (this warp + what others published)
-  float scr[68];                   // slow path: the flagged lane's group state, broadcast through shared memory;
+  float scr[76];                   // slow path: the flagged lane's group state, broadcast through shared memory;
                                    // [36..64]: subtree bounds (DYPLAN_PRUNE_BOUNDS), written once per work item
   float4 ctx[(L >= CTX_SHARED_MIN_L ? L * 32 : 1)];   // (L >= CTX_SHARED_MIN_L) [l][lane] = {X2, Rm3, U1r, A0r}: node-2 context of every lane, written
                                    // by the heavy step and read by each light step (kept out of the register file)
   unsigned long long bar;          // mbarrier of the TMA copy
-  unsigned long long pad;
+  const uint32_t* gblob;           // the request's blob in global memory (approx requests: its int32 tables)
 };
 
 #ifndef CTX_SHARED_MIN_L
@@ -41,6 +41,60 @@ struct __align__(16) FWarpShared {
 constexpr int kScrC1 = 0, kScrS1 = 1, kScrAp1 = 9, kScrU1 = 17, kScrR2 = 25, kScrIdx = 34;
 // subtree bounds: on/off, largest factor of nodes 2, 1, 0, number of (lane, node-2 sweep) pairs skipped in this item
 constexpr int kScrBnd = 36, kScrF2 = 37, kScrF1 = 38, kScrF0 = 39, kScrSkip = 40, kScrMx = 44;   // kScrMx: [node 2, 1, 0][8 levels]
+// approx requests: the flagged lane's outer digits (16 bytes) and node 2's slot, for the exact integer re-evaluation
+constexpr int kScrDig = 68, kScrSlot2 = 72;
+
+// Directed rounding.  The slack DP adds negated durations (stored rounded up) with round-up adds and
+// accumulates demands (stored rounded down) with round-down adds.  When every sum stays below 2^23 nothing rounds and
+// the slacks, T and the cap tests are exact (ReqHdr.approx = 0); beyond that each slack the screen forms is an UPPER
+// bound of the true one, so a feasible plan is never screened out and what passes is verified with integers.
+// The exact instantiation (AX = false) uses the plain operations: every value is an integer below 2^23, no rounding
+// occurs, and the compiler keeps its freedom to contract them.
+template <bool AX> __device__ __forceinline__ float addu(float a, float b) { return AX ? __fadd_ru(a, b) : a + b; }
+template <bool AX> __device__ __forceinline__ float addd(float a, float b) { return AX ? __fadd_rd(a, b) : a + b; }
+template <bool AX> __device__ __forceinline__ float subu(float a, float b) { return AX ? __fsub_ru(a, b) : a - b; }
+template <bool AX> __device__ __forceinline__ float fmau(float a, float b, float c) { return AX ? __fmaf_ru(a, b, c) : fmaf(a, b, c); }
+template <bool AX> __device__ __forceinline__ float addu_sat(float a, float b) {
+  if (!AX) return __saturatef(a + b);
+  float r;
+  asm("add.rp.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+  return r;
+}
+
+// Exact re-evaluation of one plan at one level from the int32 tables of an `approx` request: slack DP of Eq.(3) over
+// all nodes and per-backend demand sums, as plain integers.  The plan: outer digits and node 2's slot from the flagged
+// lane's scratch, node 1's and node 0's slots given.  Returns feasibility; *T_out = critical-path latency.
+template <int L>
+__device__ __forceinline__ bool exact_check(const FWarpShared<L>* __restrict__ ws, int slot1, int slot0, int l, int* T_out) {
+  const uint32_t* sb = ws->blob;
+  const ReqHdr* h = (const ReqHdr*)sb;
+  const int nsp = h->nslots_pad, Np = h->n_int;
+  const int* ilat = (const int*)(ws->gblob + h->ioff);   // [slot][L], global memory (rarely read)
+  const int* idem = ilat + nsp * L;                      // [slot]
+  const int* s_be = (const int*)(sb + kHdrWords) + nsp * (L + 2);
+  const unsigned char* sdig = (const unsigned char*)&ws->scr[kScrDig];
+  const int slo = h->slo_c;
+  int u[16], D[8];
+#pragma unroll
+  for (int b = 0; b < 8; b++) D[b] = 0;
+  int ms = slo;
+  for (int i = Np - 1; i >= 0; --i) {
+    const int slot = i >= 3 ? h->optbase[i] + sdig[i] : (i == 2 ? ((const int*)ws->scr)[kScrSlot2] : (i == 1 ? slot1 : slot0));
+    int m = slo;
+    for (uint32_t dm = h->deps[i]; dm; dm &= dm - 1) m = min(m, u[__ffs(dm) - 1]);
+    const int v = m - ilat[slot * L + l];
+    u[i] = v;
+    ms = min(ms, v);
+    const int be = s_be[slot] & 7, dmd = idem[slot];
+#pragma unroll
+    for (int b = 0; b < 8; b++) D[b] += (b == be) ? dmd : 0;
+  }
+  bool ok = ms >= 0;
+#pragma unroll
+  for (int b = 0; b < 8; b++) ok = ok && D[b] <= h->cap[b];
+  *T_out = slo - ms;
+  return ok;
+}
 
 // Loop nest of one lane over `steps` outer indices (digits of internal nodes >= 2, odometer order).  Every lane of
 // the warp runs the same number of steps (a lane whose own range is shorter keeps walking with C = 0, which can
@@ -53,7 +107,9 @@ constexpr int kScrBnd = 36, kScrF2 = 37, kScrF1 = 38, kScrF0 = 39, kScrSkip = 40
 //   slow path   (any lane saw z > 0)    for each flagged lane: its group state goes to shared memory, the 32 lanes
 //                                       re-evaluate the K0P x L (plan, level) pairs one per lane with the exact
 //                                       order 7 (T and the canonical index), candidates update the warp's incumbent
-template <int L, int K0P, int NB>
+// AX: the request is `approx` (the integer verification is compiled in; it costs the exact instantiation's enumeration
+// loop 6 % through register allocation when present, hence a template parameter and not a run-time test).
+template <int L, int K0P, int NB, bool AX>
 __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned long long o_begin, unsigned long long my_count,
                                     unsigned long long steps, int* g_thr, const int Lr, unsigned* __restrict__ slow_io) {
   constexpr int NBX = NB ? NB : 1;
@@ -73,6 +129,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
   const int Np = h->n_int, K1 = h->K1, K2 = h->Kp[2];
   const int ob2 = h->optbase[2];
   const float slo = h->slo_f, S01 = h->S01, rS01 = 1.0f / h->S01, big12 = h->big12, big02 = h->big02;
+  constexpr bool approx = AX;
   const uint32_t deps0 = h->deps[0], deps1 = h->deps[1], deps2 = h->deps[2];
 
   // inner tables in registers
@@ -143,7 +200,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       }
 #pragma unroll
       for (int l = 0; l < L; l++) {
-        const float v = m[l] + s_nlat[slot * L + l];
+        const float v = addu<AX>(m[l], s_nlat[slot * L + l]);
         u[i][l] = v;
         Rm[i][l] = fminf(Rm[i + 1][l], v);
       }
@@ -152,7 +209,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
         const int be = s_be[slot];
         const float dm = s_dem[slot];
 #pragma unroll
-        for (int b = 0; b < NBX; b++) Dp[i][b] = Dp[i + 1][b] + (be == b ? dm : 0.0f);
+        for (int b = 0; b < NBX; b++) Dp[i][b] = addd<AX>(Dp[i + 1][b], be == b ? dm : 0.0f);
       }
     }
     // ---- subtree bound (DYPLAN_PRUNE_BOUNDS; items whose lanes are in phase, so these branches are warp-uniform) ----
@@ -204,7 +261,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int l = 0; l < L; l++) {
         const float* mx = &ws->scr[kScrMx + l];   // largest negated duration of nodes 2, 1, 0 at level l
-        alive = alive || (((lvl_alive >> l) & 1u) && X2[l] + mx[0] >= 0.0f && U1r[l] + mx[8] >= 0.0f && A0r[l] + mx[16] >= 0.0f);
+        alive = alive || (((lvl_alive >> l) & 1u) && addu<AX>(X2[l], mx[0]) >= 0.0f && addu<AX>(U1r[l], mx[8]) >= 0.0f && addu<AX>(A0r[l], mx[16]) >= 0.0f);
       }
       bskip = !__any_sync(0xffffffffu, alive);
     }
@@ -267,12 +324,12 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
     for (int l = 0; l < L; l++) {
       float4 c4;
       if (kCtxShared) c4 = c4v[l]; else c4 = make_float4(X2r[l], Rm3r[l], U1rr[l], A0rr[l]);
-      const float u2 = c4.x + s_nlat[slot2 * L + l];
+      const float u2 = addu<AX>(c4.x, s_nlat[slot2 * L + l]);
       R2[l] = fminf(c4.y, u2);
-      const float U1 = fminf(c4.z, u2 + big12);
-      const float a0 = fminf(c4.w, u2 + big02);
-      A0q1[l] = fminf(a0 + 1.0f, fmaf(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
-      U1pS[l] = fmaf(U1, S01, S01);                            // (U1 + 1) * S01
+      const float U1 = fminf(c4.z, addu<AX>(u2, big12));
+      const float a0 = fminf(c4.w, addu<AX>(u2, big02));
+      A0q1[l] = fminf(addu<AX>(a0, 1.0f), fmau<AX>(R2[l], kBigF, kBigF));   // a node >= 2 misses the SLO  =>  bound <= 0
+      U1pS[l] = fmau<AX>(U1, S01, S01);                                      // (U1 + 1) * S01
     }
     const float C2 = live ? C3 * s_f[slot2] : 0.0f;   // a lane past its own range scores nothing
     float sD2[NBX];   // cap slack + 1 before nodes 1 and 0
@@ -280,7 +337,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       const int be2 = s_be[slot2];
       const float dm2 = s_dem[slot2];
 #pragma unroll
-      for (int b = 0; b < NBX; b++) sD2[b] = (capf[b] - (D3[b] + (be2 == b ? dm2 : 0.0f))) + 1.0f;
+      for (int b = 0; b < NBX; b++) sD2[b] = addu<AX>(subu<AX>(capf[b], addd<AX>(D3[b], be2 == b ? dm2 : 0.0f)), 1.0f);
     }
 
     float zm = 0.0f, zm2 = 0.0f;   // with caps: two max chains (measured: better with caps, worse without)
@@ -297,12 +354,12 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
       if (NB) {
         float smin = kBigF;
 #pragma unroll
-        for (int b = 0; b < NBX; b++) { s1[b] = sD2[b] - pd1[b]; smin = fminf(smin, s1[b]); }
+        for (int b = 0; b < NBX; b++) { s1[b] = subu<AX>(sD2[b], pd1[b]); smin = fminf(smin, s1[b]); }
         C1 *= __saturatef(smin);   // a backend is already over its cap: no plan of this group can be a candidate
       }
       float ap1[L];
 #pragma unroll
-      for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmaf(pn1[l], S01, U1pS[l]));
+      for (int l = 0; l < L; l++) ap1[l] = fminf(A0q1[l], fmau<AX>(pn1[l], S01, U1pS[l]));
       // ---- screen: K0P x L evaluations ----
       float zodd = 0.0f;             // odd L: the last level of an even k0 waits for the one of k0 + 1 (one FMNMX3 for both)
       float addend[L];
@@ -318,10 +375,10 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
 #pragma unroll
       for (int k0 = 0; k0 < K0P; k0++) {
         float P = kQuot ? f0[k0] : C1 * f0[k0];
-        if (NB) P *= __saturatef(s1[k0 / G] + ndem0[k0]);
+        if (NB) P *= addu_sat<AX>(s1[k0 / G], ndem0[k0]);
         float z[L];
 #pragma unroll
-        for (int l = 0; l < L; l++) z[l] = fmaf(__saturatef(ap1[l] + nd0[k0][l]), P, addend[l]);
+        for (int l = 0; l < L; l++) z[l] = fmaf(addu_sat<AX>(ap1[l], nd0[k0][l]), P, addend[l]);
 #pragma unroll
         for (int l = 0; l + 1 < L; l += 2) {
           if (NB && (((l >> 1) + k0) & 1)) zm2 = fmaxf(zm2, fmaxf(z[l], z[l + 1]));
@@ -352,7 +409,13 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
           for (int l = 0; l < L; l++) {
             ws->scr[kScrAp1 + l] = A0q1[l]; ws->scr[kScrU1 + l] = U1pS[l];
             // R2 is only needed here: with the context in shared memory it is re-derived instead of being kept live
-            ws->scr[kScrR2 + l] = kCtxShared ? fminf(cx[l * 32].y, cx[l * 32].x + s_nlat[slot2 * L + l]) : R2[l];
+            ws->scr[kScrR2 + l] = kCtxShared ? fminf(cx[l * 32].y, addu<AX>(cx[l * 32].x, s_nlat[slot2 * L + l])) : R2[l];
+          }
+          if (approx) {   // the exact re-evaluation needs the lane's whole plan prefix
+#pragma unroll
+            for (int w4 = 0; w4 < 4; w4++)
+              ((uint32_t*)ws->scr)[kScrDig + w4] = (uint32_t)dig[4 * w4] | ((uint32_t)dig[4 * w4 + 1] << 8) | ((uint32_t)dig[4 * w4 + 2] << 16) | ((uint32_t)dig[4 * w4 + 3] << 24);
+            ((int*)ws->scr)[kScrSlot2] = slot2;
           }
         }
         __syncwarp();
@@ -366,7 +429,7 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
           if (NB) {
             float smin = kBigF;
 #pragma unroll
-            for (int b = 0; b < NBX; b++) smin = fminf(smin, ws->scr[kScrS1 + b] - s_dem1b[k1 * 8 + b]);
+            for (int b = 0; b < NBX; b++) smin = fminf(smin, subu<AX>(ws->scr[kScrS1 + b], s_dem1b[k1 * 8 + b]));
             gC1 = __fmul_rn(gC1, __saturatef(smin));
           }
           for (int e0 = 0; e0 < K0P * L; e0 += 32) {
@@ -378,15 +441,24 @@ __device__ __noinline__ void frange(FWarpShared<L>* __restrict__ ws, unsigned lo
               k0 = e / L;
               l = e - k0 * L;
               P = __fmul_rn(gC1, s_f[k0]);
-              if (NB) P = __fmul_rn(P, __saturatef((ws->scr[kScrS1 + k0 / G] - s_dem1b[k1 * 8 + k0 / G]) - s_dem[k0]));
-              const float u1pS = fmaf(s_nlat[slot1 * L + l], S01, ws->scr[kScrU1 + l]);
-              const float t1 = fminf(ws->scr[kScrAp1 + l], u1pS) + s_nlat[e];   // slack + 1 of node 0's path
-              const float ms1 = fminf(fminf(t1, u1pS * rS01), ws->scr[kScrR2 + l] + 1.0f);   // least slack + 1
-              T = (int)((slo + 1.0f) - ms1);
+              if (NB) P = __fmul_rn(P, addu_sat<AX>(subu<AX>(ws->scr[kScrS1 + k0 / G], s_dem1b[k1 * 8 + k0 / G]), -s_dem[k0]));
+              const float u1pS = fmau<AX>(s_nlat[slot1 * L + l], S01, ws->scr[kScrU1 + l]);
+              const float t1 = addu<AX>(fminf(ws->scr[kScrAp1 + l], u1pS), s_nlat[e]);   // slack + 1 of node 0's path
+              const float ms1 = fminf(fminf(t1, u1pS * rS01), addu<AX>(ws->scr[kScrR2 + l], 1.0f));   // least slack + 1
+              // exact requests: every quantity is an integer below 2^23, T is exact.  approx requests: ms1 is an upper
+              // bound of the least slack, so this T is a LOWER bound; it is replaced by the exact one below
+              T = AX ? (int)fminf(fmaxf(__fsub_rd(__fadd_rd(slo, 1.0f), ms1), 0.0f), 2147483520.0f) : (int)((slo + 1.0f) - ms1);
               // phase 1: feasible, and not worse than the warp's incumbent on (C desc, T asc)
               const float bC = ((volatile float*)&ws->best[l].C)[0];
               const int bT = ((volatile int*)&ws->best[l].T)[0];
               cand = P > 0.0f && t1 >= 1.0f && (P > bC || (P == bC && T <= bT)) && P >= __int_as_float(((volatile int*)w_thr)[l]);
+              if (AX && cand) {
+                // the conservative test passed: now the plan's exact latency, SLO and caps in integers
+                int Tx = 0;
+                const bool ok = exact_check<L>(ws, slot1, k0, l, &Tx);
+                T = Tx;
+                cand = ok && (P > bC || (P == bC && T <= bT));
+              }
             }
             unsigned cm = __ballot_sync(0xffffffffu, cand);
             if (cm && !have_idx) {
@@ -487,6 +559,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
         const uint32_t words = (uint32_t)__ldg(&((const ReqHdr*)gblob)->blob_words);
         tma_load_1d(ws->blob, gblob, words * 4u, &ws->bar);
       }
+      if (lane == 0) ws->gblob = gblob;
       mbar_wait(&ws->bar, phase);
       phase ^= 1;
       cur_req = r;
@@ -537,7 +610,8 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
       const unsigned long long n = te - tb;
       const unsigned long long t0 = n ? tb : 0ull;   // an idle lane walks from outer index 0 (with C = 0)
       switch (h->nbc * 32 + h->K0p) {
-#define DYPLAN_FCASE(NB_, K_) case NB_ * 32 + K_: frange<L, K_, NB_>(ws, t0, n, per, g_thr, Lr, &slow_steps); break;
+#define DYPLAN_FCASE(NB_, K_) case NB_ * 32 + K_: if (h->approx) frange<L, K_, NB_, true>(ws, t0, n, per, g_thr, Lr, &slow_steps); \
+                                                  else frange<L, K_, NB_, false>(ws, t0, n, per, g_thr, Lr, &slow_steps); break;
         DYPLAN_FCASE(0, 2) DYPLAN_FCASE(0, 4) DYPLAN_FCASE(0, 6) DYPLAN_FCASE(0, 8) DYPLAN_FCASE(0, 12) DYPLAN_FCASE(0, 16)
         DYPLAN_FCASE(2, 2) DYPLAN_FCASE(2, 4) DYPLAN_FCASE(2, 6) DYPLAN_FCASE(2, 8) DYPLAN_FCASE(2, 12) DYPLAN_FCASE(2, 16)
         DYPLAN_FCASE(3, 6) DYPLAN_FCASE(3, 12)

@@ -10,7 +10,7 @@ namespace dyplan {
 
 constexpr int kBlock = 128;          // threads per scoring block
 constexpr int kMinBlocks = 4;        // resident scoring blocks per SM the register allocation is bounded for
-constexpr int kHdrWords = 120;       // ReqHdr size in 4-byte words (multiple of 4 -> 16-byte aligned tables)
+constexpr int kHdrWords = 124;       // ReqHdr size in 4-byte words (multiple of 4 -> 16-byte aligned tables)
 constexpr int kMaxSlots = 16 * 16 + 4;  // option slots of one request incl. dummies, padded to 4
 constexpr int kDem0bWords = 16 * 8;  // per-backend demand of the inner node's options [k0][b]
 constexpr int kMaxBlobWords = kHdrWords + kDem0bWords + kMaxSlots * (DYPLAN_MAX_LEVELS + 3);
@@ -19,11 +19,12 @@ constexpr int kMaxBlobWords = kHdrWords + kDem0bWords + kMaxSlots * (DYPLAN_MAX_
 __host__ __device__ inline size_t blob_stride_words(int L) { return (size_t)kHdrWords + kDem0bWords + (size_t)kMaxSlots * (size_t)(L + 3); }
 constexpr uint64_t kNoIdx = ~0ull;
 constexpr int kClassWide = 0;        // int32 slack DP (k_score): any request the ABI admits
-constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): every latency / demand sum below 2^22, tables <= kFastBlobWords
+constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): exact when every latency / demand sum is below 2^22, else a
+                                     // conservative screen whose candidates are verified in int32 (ReqHdr.approx); tables <= kFastBlobWords
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
 constexpr uint32_t kFastItemsPerWarp = 12;   // work items to aim for per resident warp (measured: 8 and 24 lose 4-7 % on cfg4)
-constexpr float kBigF = 16777216.0f; // 2^24
+constexpr float kBigF = 1099511627776.0f; // 2^40: above every slack, latency and demand the ABI admits (< 2^31)
 // fast class: outer indices per work item of a request whose node 2 has K2 options -- the call-wide figure rounded up
 // so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)
 __host__ __device__ inline unsigned long long fast_item_outer(unsigned long long pif, int K2, bool small_call) {
@@ -63,8 +64,14 @@ struct ReqHdr {
   float S01;             // 1 if internal node 1 is in deps(0), else 2^24 (turns "u1 >= 0" into a bound that never binds)
   float big12, big02;    // 0 if internal node 2 is in deps(1) / deps(0), else 2^24
   int32_t blob_words;    // words of this request's staged blob (header + tables)
-  float capf[8];         // min(cap, largest possible demand) per backend (+big when absent)
+  float capf[8];         // min(cap, largest possible demand) per backend (+big when absent), rounded up
   unsigned long long stride[16];   // canonical stride of internal node i (0 for dummies / pinned nodes)
+  int32_t approx;        // 1: a latency or demand sum can exceed 2^22, so the fp32 slacks are upper bounds (directed
+                         //    rounding) and every candidate is verified with the int32 tables that follow the fp32 ones
+  int32_t slo_c;         // min(SLO, longest possible T) as an integer
+  int32_t ioff;          // word offset of the int32 tables ilat[slot][Lp], idem[slot] in the request's blob in GLOBAL memory
+                         // (approx only; they follow the blob_words the scorer stages in shared memory)
+  int32_t pad1;
 };
 static_assert(sizeof(ReqHdr) == kHdrWords * 4, "ReqHdr layout");
 
@@ -90,7 +97,7 @@ struct CallState {
   uint32_t fast_requests;           // requests staged for the fp32 scorer
   uint32_t small_call_f;            // fast class: fewer than ~1K outer indices per resident warp (items are not lane-aligned)
   uint32_t tail_start_f;            // fast class: requests >= this index are cut into 4x smaller items (they are handed out last: a short tail)
-  uint32_t pad0;
+  uint32_t approx_requests;         // fast class: requests verified in int32 (ReqHdr.approx)
 };
 // outer indices per item of request r before rounding (k_plan and k_fscore must agree)
 __host__ __device__ inline unsigned long long fast_pif_of(unsigned long long pif, uint32_t tail_start, long long r) {

@@ -207,7 +207,10 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   const int Lp = level_class(L);
   const bool has_caps = b.cap != nullptr;
   const int nbc = !has_caps ? 0 : (B <= 2 ? 2 : (B == 3 ? 3 : (B == 4 ? 4 : 8)));
-  const bool fast_pre = sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)) && min_c >= 1e-30;
+  // the fp32 scorer is exact when every slack / demand sum is an integer below 2^23; beyond that its slacks are upper
+  // bounds (directed rounding) and candidates are verified with int32 tables (ReqHdr.approx)
+  const bool fast_pre = min_c >= 1e-30;
+  const bool approx = !(sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)));
   // options kept per node: all of them, or (opt-in, fast class only) the ones no other option dominates
   const uint32_t keep_full = (e >= 0 && !fixed) ? (myK >= 32 ? 0xffffffffu : ((1u << myK) - 1u)) : 1u;
   uint32_t keep = keep_full;
@@ -257,7 +260,8 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       optbase -= width;
       nslots_pad = (nslots + 3) & ~3;
       blob_words = kHdrWords + nslots_pad * (Lp + 5) + (nbc ? 128 : 0);
-      if (!(fast && (blob_words > kFastBlobWords || (size_t)blob_words > blob_stride))) break;
+      // (approx: the int32 tables follow in global memory and are not staged in the scorer's window)
+      if (!(fast && (blob_words > kFastBlobWords || (size_t)blob_words + (approx ? nslots_pad * (Lp + 1) : 0) > blob_stride))) break;
       // tables too large for the fp32 scorer's window: fall back to the wide class (lay out again, plain inner radix)
       fast = false;
       K0p = k0_class(K0r);
@@ -293,14 +297,18 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     for (int bb = 0; bb < 8; bb++) h->cap[bb] = (b.cap && bb < B) ? b.cap[r * B + bb] : INT32_MAX;
     h->klass = fast ? kClassFast : kClassWide; h->nbc = fast ? nbc : 0; h->Lp = Lp;
     const long long slo = b.slo_us[r];
-    h->slo_f = (float)(slo < sum_lat ? slo : sum_lat);
+    h->slo_f = __ll2float_ru(slo < sum_lat ? slo : sum_lat);
+    h->slo_c = (int32_t)(slo < sum_lat ? slo : sum_lat);
+    h->approx = (fast && approx) ? 1 : 0;
+    h->ioff = kHdrWords + nslots_pad * (Lp + 5) + (nbc ? 128 : 0);
+    h->pad1 = 0;
     h->S01 = ((deps0 >> 1) & 1) ? 1.0f : kBigF;
     h->big12 = ((deps1 >> 2) & 1) ? 0.0f : kBigF;
     h->big02 = ((deps0 >> 2) & 1) ? 0.0f : kBigF;
     h->blob_words = fast ? blob_words : 0;
     for (int bb = 0; bb < 8; bb++) {
       long long c = (b.cap && bb < B) ? (long long)b.cap[r * B + bb] : sum_dem;
-      h->capf[bb] = (float)(c < sum_dem ? c : sum_dem);
+      h->capf[bb] = __ll2float_ru(c < sum_dem ? c : sum_dem);
     }
   }
   if (lane < 16) {
@@ -324,6 +332,8 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   int* q_be = (int*)(q_dem + nslots_pad);
   unsigned long long* q_idxc = (unsigned long long*)(q_be + nslots_pad);
   float* q_dem1b = (float*)(q_idxc + nslots_pad);
+  int* q_ilat = (int*)(q_dem1b + (nbc ? 128 : 0));   // approx only: exact durations [slot][Lp] and demands [slot]
+  int* q_idem = q_ilat + nslots_pad * Lp;
   if (!fast) for (int i = lane; i < kDem0bWords; i += 32) t_dem0b[i] = 0;
   else if (nbc) for (int i = lane; i < 128; i += 32) q_dem1b[i] = 0.0f;
   __syncwarp();
@@ -388,10 +398,17 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     if (active && fast) {
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
-        if (l < Lp) q_nlat[s * Lp + l] = pad ? -2.0f * kBigF : -(float)dl[l < L ? l : 0];   // padded levels repeat level 0 (their threshold never admits a plan)
-      q_f[s] = pad ? 0.0f : f; q_dem[s] = (float)dem; q_be[s] = be;
+        if (l < Lp) q_nlat[s * Lp + l] = pad ? -2.0f * kBigF : __int2float_ru(-dl[l < L ? l : 0]);   // padded levels repeat level 0 (their threshold never admits a plan)
+      // (negated durations rounded up and demands rounded down: exact below 2^24, else the slacks formed from them
+      // are upper bounds)
+      q_f[s] = pad ? 0.0f : f; q_dem[s] = __int2float_rd(dem); q_be[s] = be;
       q_idxc[s] = (pad || ne < 0 || nfix) ? 0ull : (unsigned long long)korig * nstride;
-      if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = (float)dem;
+      if (nbc && node == 1 && !pad) q_dem1b[k * 8 + be] = __int2float_rd(dem);
+      if (approx) {
+#pragma unroll
+        for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) if (l < Lp) q_ilat[s * Lp + l] = dl[l < L ? l : 0];
+        q_idem[s] = dem;
+      }
     }
   }
 }
@@ -418,45 +435,52 @@ __global__ void __launch_bounds__(kSeedThreads) k_seed(CallArgs a) {
   const float* p_f = p_nlat + nsp * Lp;
   const float* p_dem = p_f + nsp;
   const int* p_be = (const int*)(p_dem + nsp);
-  const float slo_f = sh->slo_f;
-  float su[16][DYPLAN_MAX_LEVELS];
+  // feasibility is decided on integers in both sub-classes (exact: the fp32 tables hold integers below 2^23 and
+  // convert exactly; approx: the int32 tables that follow them), so a threshold is always the C32 of a feasible plan
+  const bool approx = sh->approx != 0;
+  const int* p_ilat = (const int*)(blob + sh->ioff);   // (global memory: not part of blob_words)
+  const int* p_idem = p_ilat + nsp * Lp;
+  const int slo_c = sh->slo_c;
+  int su[16][DYPLAN_MAX_LEVELS];
   for (int sidx = 0; sidx < kSeedsPerThread; sidx++) {
     uint32_t x = (uint32_t)r * 0x9E3779B9u + (uint32_t)(sidx * kSeedThreads + tid) * 0x85EBCA6Bu + 0x27D4EB2Fu;
-    float C = 1.0f, D[8], ms[DYPLAN_MAX_LEVELS];
+    float C = 1.0f;
+    int D[8], ms[DYPLAN_MAX_LEVELS];
 #pragma unroll
-    for (int i = 0; i < 8; i++) D[i] = 0.0f;
+    for (int i = 0; i < 8; i++) D[i] = 0;
 #pragma unroll
-    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) ms[l] = slo_f;
+    for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) ms[l] = slo_c;
     for (int i = Np - 1; i >= 0; --i) {
       x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;   // integer hash, one draw per node
       const int kp = i == 0 ? K0p : sh->Kp[i];
       const int slot = sh->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
       C *= p_f[slot];
       const int be = p_be[slot] & 7;
-      const float dm = p_dem[slot];
+      const int dm = approx ? p_idem[slot] : (int)p_dem[slot];
 #pragma unroll
-      for (int bb = 0; bb < 8; bb++) D[bb] += (bb == be) ? dm : 0.0f;
+      for (int bb = 0; bb < 8; bb++) D[bb] += (bb == be) ? dm : 0;
       const uint32_t dm0 = sh->deps[i];
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
         if (l < L) {
-          float m = slo_f;
-          for (uint32_t dmk = dm0; dmk; dmk &= dmk - 1) m = fminf(m, su[__ffs(dmk) - 1][l]);
-          const float v = m + p_nlat[slot * Lp + l];
+          int m = slo_c;
+          for (uint32_t dmk = dm0; dmk; dmk &= dmk - 1) m = min(m, su[__ffs(dmk) - 1][l]);
+          const int d = approx ? p_ilat[slot * Lp + l] : (int)(-p_nlat[slot * Lp + l]);   // (padding slot: 2^41 saturates, C = 0 anyway)
+          const int v = m - d;
           su[i][l] = v;
-          ms[l] = fminf(ms[l], v);
+          ms[l] = min(ms[l], v);
         }
       }
     }
     bool capok = C > 0.0f;   // a padding slot of node 0 has f = 0
     if (nbc) {
 #pragma unroll
-      for (int bb = 0; bb < 8; bb++) capok &= (bb >= B) || D[bb] <= sh->capf[bb];
+      for (int bb = 0; bb < 8; bb++) capok &= (bb >= B) || D[bb] <= sh->cap[bb];
     }
     if (capok) {
 #pragma unroll
       for (int l = 0; l < DYPLAN_MAX_LEVELS; l++)
-        if (l < L && ms[l] >= 0.0f) atomicMax((int*)&a.gthr[r * L + l], __float_as_int(C));
+        if (l < L && ms[l] >= 0) atomicMax((int*)&a.gthr[r * L + l], __float_as_int(C));
     }
   }
 }
@@ -488,22 +512,23 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   const long long chunk = (R + 1023) / 1024;
   const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
   unsigned long long so = 0, sf = 0, sp = 0, mxf = 0;
-  uint32_t nf = 0;
+  uint32_t nf = 0, na = 0;
+  __shared__ uint32_t s_na[1024];
   __shared__ unsigned long long s_mxf;
   if (tid == 0) s_mxf = 0;
   __syncthreads();
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     if (h->status == DYPLAN_ST_OK) {
-      if (h->klass == kClassFast) { sf += h->outer_total; nf++; mxf = h->outer_total > mxf ? h->outer_total : mxf; } else so += h->outer_total;
+      if (h->klass == kClassFast) { sf += h->outer_total; nf++; na += h->approx ? 1u : 0u; mxf = h->outer_total > mxf ? h->outer_total : mxf; } else so += h->outer_total;
       sp += h->outer_total * (unsigned long long)(h->K0 * h->K1);
     }
   }
-  s_sum[tid] = so; s_sumf[tid] = sf; s_plans[tid] = sp; s_nf[tid] = nf;
+  s_sum[tid] = so; s_sumf[tid] = sf; s_plans[tid] = sp; s_nf[tid] = nf; s_na[tid] = na;
   if (mxf) atomicMax(&s_mxf, mxf);
   __syncthreads();
   for (int off = 512; off; off >>= 1) {
-    if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_sumf[tid] += s_sumf[tid + off]; s_plans[tid] += s_plans[tid + off]; s_nf[tid] += s_nf[tid + off]; }
+    if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_sumf[tid] += s_sumf[tid + off]; s_plans[tid] += s_plans[tid + off]; s_nf[tid] += s_nf[tid + off]; s_na[tid] += s_na[tid + off]; }
     __syncthreads();
   }
   const unsigned long long total_w = s_sum[0], total_f = s_sumf[0], total_plans = s_plans[0];
@@ -564,7 +589,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
     st->slow_steps = 0; st->bound_skipped = 0;
     st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
-    st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u; st->tail_start_f = tail_start; st->pad0 = 0;
+    st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u; st->tail_start_f = tail_start; st->approx_requests = s_na[0];
   }
 }
 

@@ -210,24 +210,69 @@ def _scale_latencies(w, rows, factor):
         b.slo_us[r] = int(min(int(b.slo_us[r]) * factor, 2**31 - 1))
 
 
-@pytest.mark.parametrize("seed,L,B,caps", [(91, 2, 2, True), (92, 4, 3, False), (93, 5, 4, True)])
-def test_wide_class_large_latencies(dy, orc, seed, L, B, caps):
-    # latency sums far above 2^22 us: not exact in fp32, so every request goes to the int32 scorer
-    w = wl.random_workload(seed, R=24, nmin=2, nmax=7, kmin=1, kmax=6, B=B, M=3, L=L, caps=caps)
-    _scale_latencies(w, range(w.batch.R), 3000)
+@pytest.mark.parametrize("seed,L,B,caps,factor", [(91, 2, 2, True, 3000), (92, 4, 3, False, 3000), (93, 5, 4, True, 3000),
+                                                  (191, 3, 2, True, 40000), (192, 8, 3, False, 40000), (193, 1, 1, True, 40000)])
+def test_large_latencies_take_the_verified_fp32_path(dy, orc, seed, L, B, caps, factor):
+    # latency sums far above 2^22 us (the paper's own requests take 4 s ... 414 s): fp32 is no longer exact, so
+    # the fp32 scorer runs as a conservative screen (slack upper bounds by directed rounding) and every candidate is
+    # re-evaluated in int32 (ReqHdr.approx).  Factor 40000 puts durations near 2^27 (fp32 spacing 8-16 us): the SLO is
+    # some sampled plan's exact T, so plans sit exactly on and next to the feasibility boundary.
+    nmax = 7 if factor == 3000 else 5
+    w = wl.random_workload(seed, R=24, nmin=2, nmax=nmax, kmin=1, kmax=6, B=B, M=3, L=L, caps=caps)
+    _scale_latencies(w, range(w.batch.R), factor)
+    if caps and factor != 3000:   # demand sums beyond 2^22 as well
+        w.batch.demand[:] = w.batch.demand.astype(np.int64) * 5000
+        w.batch.cap[:] = np.minimum(w.batch.cap.astype(np.int64) * 5000, 2**31 - 1).astype(np.int32)
     g = gpu_run(dy, w)
     st = dy[1].dyplan_last_stats()
-    assert st["fast_requests"] <= 2        # (a one- or two-node request can still fit under 2^22)
-    check_records(orc, w, g, orc.run(w), where=f"wide-class(seed={seed})")
+    assert st["fast_requests"] == w.batch.R
+    assert st["approx_requests"] >= w.batch.R - 2        # (a one- or two-node request can still fit under 2^22)
+    ref = orc.run(w)
+    assert (ref["status"] == 0).sum() > 10
+    check_records(orc, w, g, ref, where=f"verified-fp32(seed={seed})")
+
+
+def test_verified_fp32_path_on_the_feasibility_boundary(dy, orc):
+    # SLO = T of the oracle's own optimum, SLO - 1 and SLO + 1, with durations around 2^28: the screen's rounded slacks
+    # cannot tell these apart, the integer verification must
+    w = wl.random_workload(194, R=12, nmin=3, nmax=5, kmin=2, kmax=5, B=2, M=2, L=2, caps=False, tool_p=0.0)
+    _scale_latencies(w, range(w.batch.R), 60000)
+    ref0 = orc.run(w)
+    for delta in (0, -1, 1):
+        for r in range(w.batch.R):
+            if ref0["status"][r * 2] == 0:
+                w.batch.slo_us[r] = int(ref0["lat"][r * 2]) + delta
+        g = gpu_run(dy, w)
+        assert dy[1].dyplan_last_stats()["approx_requests"] >= 10
+        check_records(orc, w, g, orc.run(w), where=f"boundary(delta={delta})")
 
 
 def test_mixed_classes_in_one_batch(dy, orc):
     w = wl.random_workload(94, R=40, nmin=2, nmax=7, kmin=1, kmax=6, B=2, M=3, L=3, caps=True)
     _scale_latencies(w, range(0, 40, 3), 3000)
+    b = w.batch
+    for r in range(1, 40, 6):      # and some requests only the int32 scorer takes (a zero factor)
+        n = int(b.node_off[r])
+        b.vuln[n] = 1.0
+        b.acc[int(b.opt_off[n]): int(b.opt_off[n + 1])] = 0.0
     g = gpu_run(dy, w)
     st = dy[1].dyplan_last_stats()
-    assert 0 < st["fast_requests"] < w.batch.R
+    assert 0 < st["approx_requests"] < st["fast_requests"] < w.batch.R
     check_records(orc, w, g, orc.run(w), where="mixed-classes")
+
+
+def test_int32_scorer_with_large_latencies(dy, orc):
+    # the wide class proper: zero factors AND second-scale latencies
+    w = wl.random_workload(195, R=16, nmin=2, nmax=6, kmin=2, kmax=5, B=2, M=2, L=3, caps=True, tool_p=0.0)
+    _scale_latencies(w, range(w.batch.R), 3000)
+    b = w.batch
+    for r in range(16):
+        n = int(b.node_off[r]) + (r % b.n_nodes(r))
+        b.vuln[n] = 1.0
+        b.acc[int(b.opt_off[n])] = 0.0          # one zero-factor option: the request leaves the fp32 scorer
+    g = gpu_run(dy, w)
+    assert dy[1].dyplan_last_stats()["fast_requests"] == 0
+    check_records(orc, w, g, orc.run(w), where="int32-scorer")
 
 
 def test_zero_factor_requests_go_to_the_int32_scorer(dy, orc):
