@@ -124,6 +124,11 @@ typedef struct {
  *   Exact: results are those of the full enumeration (parity-tested against the unpruned oracle).  dyplan_stats.plans
  *   still counts the whole space; dyplan_stats.bound_skipped counts the outer indices that were not walked. */
 #define DYPLAN_PRUNE_BOUNDS 2u
+/* DYPLAN_NO_SMALL_PATH: by default a call of at most 32 requests hands every request with at most 2^21 (plan, level)
+ *   evaluations to a latency-oriented kernel (one admission-time compile: PAPER.md:211) that scores each plan from
+ *   scratch in int32 with no incumbent seeds, work items or persistent grid; records are identical.  This flag sends
+ *   every request through the batched scorers instead (used by the tests to compare the two paths). */
+#define DYPLAN_NO_SMALL_PATH 4u
 
 /* Create / destroy a context on CUDA device `device_ordinal`.  Fails (DYPLAN_ERR_CUDA) without a device. */
 DYPLAN_API int dyplan_create(dyplan_ctx** out, int device_ordinal);
@@ -276,6 +281,8 @@ typedef struct {
   uint64_t bound_skipped; /* outer indices (assignments of all but the two innermost digits) skipped by DYPLAN_PRUNE_BOUNDS */
   uint64_t approx_requests; /* of fast_requests: those whose latency or demand sums exceed 2^22, scored by the fp32 kernel as a
                                conservative screen with every candidate verified in int32 (results identical)          */
+  uint64_t small_requests;  /* requests solved by the small-call kernel (calls of at most 32 requests: every request with at
+                               most 2^21 (plan, level) evaluations); they are in neither fast_requests nor work_items     */
 } dyplan_stats;
 /* Synchronises `stream` of the last call, then fills *out. */
 DYPLAN_API int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out);

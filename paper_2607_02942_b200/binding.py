@@ -52,6 +52,7 @@ class CBundle(C.Structure):
 
 PRUNE_DOMINATED = 1
 PRUNE_BOUNDS = 2
+NO_SMALL_PATH = 4
 
 
 class CSwitchParams(C.Structure):
@@ -76,7 +77,7 @@ class CProfiles(C.Structure):
 class CStats(C.Structure):
     _fields_ = [("plans", C.c_uint64), ("evals", C.c_uint64), ("work_items", C.c_uint64), ("slow_steps", C.c_uint64),
                 ("fast_requests", C.c_uint64), ("launches", C.c_int32), ("sm_count", C.c_int32), ("score_ms", C.c_float),
-                ("bound_skipped", C.c_uint64), ("approx_requests", C.c_uint64)]
+                ("bound_skipped", C.c_uint64), ("approx_requests", C.c_uint64), ("small_requests", C.c_uint64)]
 
 
 class CIssueRate(C.Structure):
@@ -256,6 +257,7 @@ class Context:
             self._h = C.c_void_p()
             raise DyplanError(rc, dyplan_strerror(rc) + " (dyplan_create: no usable CUDA device?)")
         self.device_ordinal = device_ordinal
+        self.flags = 0
 
     def close(self):
         if self._h:
@@ -321,6 +323,7 @@ class Context:
 
     def dyplan_set_flags(self, flags: int):
         self._check(lib().dyplan_set_flags(self._h, int(flags)))
+        self.flags = int(flags)
 
     def dyplan_switch(self, batch: Buffers, bundle: Buffers, L: int, params: dict, model_load, since_switch,
                       dispatched_mask, cur_variant, active_choice, switched, stream=None):

@@ -68,6 +68,8 @@ struct dyplan_ctx {
   uint32_t flags = 0;
   // staging for the *_host calls: one device arena, one pinned-or-not host side is the caller's
   DevBuf arena;
+  void* hstage = nullptr;          // pinned host image of the arena for small *_host calls (one copy in, one copy out)
+  size_t hstage_cap = 0;
   // occupancy cache [L-1][nb index]
   int occ[8][4];
   int focc[8];
@@ -140,7 +142,7 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
 
 int dyplan_set_flags(dyplan_ctx* ctx, uint32_t flags) {
   if (!ctx) return DYPLAN_ERR_NULL;
-  if (flags & ~(DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS)) return DYPLAN_ERR_ARG;
+  if (flags & ~(DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS | DYPLAN_NO_SMALL_PATH)) return DYPLAN_ERR_ARG;
   ctx->flags = flags;
   return DYPLAN_OK;
 }
@@ -151,6 +153,7 @@ int dyplan_destroy(dyplan_ctx* ctx) {
   DevBuf* bufs[] = {&ctx->blob, &ctx->item_off, &ctx->done, &ctx->gthr, &ctx->partial, &ctx->state, &ctx->arena,
                     &ctx->lin_blob, &ctx->lin_gj, &ctx->lin_gkey, &ctx->lin_misc};
   for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
+  if (ctx->hstage) cudaFreeHost(ctx->hstage);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
   delete ctx;
@@ -179,8 +182,11 @@ static int check_bundle(const dyplan_bundle* o) {
 }
 
 // compile and replan share everything but two arguments
+// all_small: the caller (a *_host entry point, which sees the option counts) has established that every request of the
+// call is one k_small takes, so the batched scorers are not launched at all
 static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult, const uint32_t* dispatched,
-                     const uint8_t* fixed_choice, uint32_t flags, bool is_replan, dyplan_bundle* out, cudaStream_t stream) {
+                     const uint8_t* fixed_choice, uint32_t flags, bool is_replan, dyplan_bundle* out, cudaStream_t stream,
+                     bool all_small = false) {
   if (!ctx) return DYPLAN_ERR_NULL;
   int rc = check_batch(in, true);
   if (rc) return rc;
@@ -230,17 +236,25 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f;
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
   a.max_items = max_items;
-
+  a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
+  a.small_split = a.small_mode ? (4 * ctx->sm_count / (int)in->R > 1 ? 4 * ctx->sm_count / (int)in->R : 1) : 1;
 
   CK(launch_stage(a, stream));
-  CK(launch_seed(a, stream));
-  CK(launch_plan(a, stream));
-  CK(cudaEventRecord(ctx->ev0, stream));
-  CK(kFLaunch[L - 1](a, fgrid, stream));      // fp32 scorer: requests of the fast class
-  CK(kLaunch[L - 1](a, nbc, grid, stream));   // int32 scorer: the rest (exits at once when it has no work items)
+  int launches = 1;
+  const bool only_small = a.small_mode && all_small;
+  if (only_small) CK(cudaEventRecord(ctx->ev0, stream));   // (score_ms: k_small here, else the batched scorers)
+  if (a.small_mode) { CK(launch_small(a, stream)); launches++; }   // small requests of a small call: solved here (admission path)
+  if (!only_small) {
+    CK(launch_seed(a, stream));
+    CK(launch_plan(a, stream));
+    CK(cudaEventRecord(ctx->ev0, stream));
+    CK(kFLaunch[L - 1](a, fgrid, stream));      // fp32 scorer: requests of the fast class
+    CK(kLaunch[L - 1](a, nbc, grid, stream));   // int32 scorer: the rest (exits at once when it has no work items)
+    launches += 4;
+  }
   CK(cudaEventRecord(ctx->ev1, stream));
   ctx->have_events = true;
-  ctx->last_launches = 5;
+  ctx->last_launches = launches;
   return DYPLAN_OK;
 }
 
@@ -460,6 +474,7 @@ int dyplan_last_stats(dyplan_ctx* ctx, dyplan_stats* out) {
     out->slow_steps = st.slow_steps;
     out->bound_skipped = st.bound_skipped;
     out->approx_requests = st.approx_requests;
+    out->small_requests = st.small_requests;
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     out->score_ms = ms;
@@ -475,6 +490,7 @@ namespace {
 struct Arena {
   char* base;
   size_t off;
+  char* stage = nullptr;   // pinned host image (small calls), else null
   template <typename T>
   T* take(size_t n) {
     off = (off + 255) & ~(size_t)255;
@@ -507,10 +523,18 @@ size_t arena_bytes(const HostPlan& p) {
 
 }  // namespace
 
+// A small call is dominated by the fixed cost of its copies (12-14 cudaMemcpyAsync in, 8 out): below kStageBytes the
+// inputs are packed into a pinned image of the arena and travel as ONE copy each way; larger calls copy each array
+// straight from the caller's buffer (packing 27 MB on the host would cost more than it saves).
+constexpr size_t kStageBytes = 256 << 10;
 #define H2D(dst, src, n, T)                                                                            \
   do {                                                                                                 \
     dst = ar.take<T>(n);                                                                               \
-    if ((n) > 0) { CK(cudaMemcpyAsync((void*)dst, src, (size_t)(n) * sizeof(T), cudaMemcpyHostToDevice, s)); h2d += (size_t)(n) * sizeof(T); } \
+    if ((n) > 0) {                                                                                     \
+      if (ar.stage) memcpy(ar.stage + ((char*)dst - ar.base), src, (size_t)(n) * sizeof(T));           \
+      else CK(cudaMemcpyAsync((void*)dst, src, (size_t)(n) * sizeof(T), cudaMemcpyHostToDevice, s));   \
+      h2d += (size_t)(n) * sizeof(T);                                                                  \
+    }                                                                                                  \
   } while (0)
 
 static int batch_to_device(dyplan_ctx* ctx, const dyplan_batch* in, Arena& ar, dyplan_batch* d, cudaStream_t s, uint64_t& h2d) {
@@ -541,10 +565,16 @@ static void bundle_alloc(Arena& ar, size_t nrec, size_t B, bool want64, dyplan_b
 
 #define D2H(dst, src, n, T)                                                                              \
   do {                                                                                                   \
-    if ((n) > 0 && (dst)) { CK(cudaMemcpyAsync((void*)(dst), src, (size_t)(n) * sizeof(T), cudaMemcpyDeviceToHost, s)); d2h += (size_t)(n) * sizeof(T); } \
+    if ((n) > 0 && (dst)) {                                                                              \
+      if (stage) memcpy((void*)(dst), stage + ((const char*)(src) - abase), (size_t)(n) * sizeof(T));    \
+      else CK(cudaMemcpyAsync((void*)(dst), src, (size_t)(n) * sizeof(T), cudaMemcpyDeviceToHost, s));   \
+      d2h += (size_t)(n) * sizeof(T);                                                                    \
+    }                                                                                                    \
   } while (0)
 
-static int bundle_to_host(dyplan_ctx* ctx, const dyplan_bundle* d, dyplan_bundle* h, size_t nrec, size_t B, cudaStream_t s, uint64_t& d2h) {
+// stage != null: the device arena's output region is already in the pinned image (one copy, synchronised): scatter it
+static int bundle_to_host(dyplan_ctx* ctx, const dyplan_bundle* d, dyplan_bundle* h, size_t nrec, size_t B, cudaStream_t s, uint64_t& d2h,
+                          const char* stage = nullptr, const char* abase = nullptr) {
   D2H(h->plan_idx, d->plan_idx, nrec, uint64_t);
   D2H(h->choice, d->choice, nrec * 16, uint8_t);
   D2H(h->corr, d->corr, nrec, float);
@@ -580,18 +610,48 @@ static int solve_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const 
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
   HostPlan hp{(size_t)in->R, (size_t)in->NN, (size_t)in->KK, (size_t)in->B, (size_t)L, (size_t)in->R * L};
-  if ((rc = ensure(ctx, ctx->arena, arena_bytes(hp)))) return rc;
+  const size_t abytes = arena_bytes(hp);
+  if ((rc = ensure(ctx, ctx->arena, abytes))) return rc;
   Arena ar{(char*)ctx->arena.p, 0};
+  if (abytes <= kStageBytes) {
+    if (ctx->hstage_cap < kStageBytes) {
+      if (ctx->hstage) CK(cudaFreeHost(ctx->hstage));
+      ctx->hstage = nullptr; ctx->hstage_cap = 0;
+      CK(cudaHostAlloc(&ctx->hstage, kStageBytes, cudaHostAllocDefault));
+      ctx->hstage_cap = kStageBytes;
+    }
+    ar.stage = (char*)ctx->hstage;
+  }
   dyplan_batch d;
   if ((rc = batch_to_device(ctx, in, ar, &d, s, h2d))) return rc;
   int32_t* dmult; uint32_t* ddisp = nullptr; uint8_t* dfix = nullptr;
   H2D(dmult, mult, is_replan ? (size_t)in->R * in->B : (size_t)L * in->B, int32_t);
   if (is_replan) { H2D(ddisp, dispatched, (size_t)in->R, uint32_t); H2D(dfix, fixed_choice, (size_t)in->NN, uint8_t); }
+  if (ar.stage) CK(cudaMemcpyAsync(ar.base, ar.stage, ar.off, cudaMemcpyHostToDevice, s));   // the whole input image, once
+  const size_t out_begin = (ar.off + 255) & ~(size_t)255;
   dyplan_bundle dout;
   bundle_alloc(ar, hp.nrec, hp.B, out->corr64 != nullptr, &dout);
-  if ((rc = run_solve(ctx, &d, L, dmult, ddisp, dfix, flags, is_replan, &dout, s))) return rc;
-  if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h))) return rc;
-  CK(cudaStreamSynchronize(s));
+  // every request small enough for k_small (an upper bound of what k_stage will find: pinned nodes only shrink it)?
+  bool all_small = in->R <= kSmallMaxR;
+  for (int32_t r = 0; r < in->R && all_small; r++) {
+    const int32_t n0 = in->node_off[r], n1 = in->node_off[r + 1];
+    if (n0 < 0 || n1 < n0 || n1 > in->NN) break;   // malformed: k_stage reports it
+    unsigned long long p = 1;
+    for (int32_t n = n0; n < n1 && all_small; n++) {
+      const long long k = (long long)in->opt_off[n + 1] - in->opt_off[n];
+      if (k >= 1 && k <= DYPLAN_MAX_OPTS) p *= (unsigned long long)k;
+      if (p * (unsigned long long)L > kSmallMaxEvals) all_small = false;
+    }
+  }
+  if ((rc = run_solve(ctx, &d, L, dmult, ddisp, dfix, flags, is_replan, &dout, s, all_small))) return rc;
+  if (ar.stage) {
+    CK(cudaMemcpyAsync(ar.stage + out_begin, ar.base + out_begin, ar.off - out_begin, cudaMemcpyDeviceToHost, s));   // every record, once
+    CK(cudaStreamSynchronize(s));
+    if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h, ar.stage, ar.base))) return rc;
+  } else {
+    if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h))) return rc;
+    CK(cudaStreamSynchronize(s));
+  }
   if (h2d_bytes) *h2d_bytes = h2d;
   if (d2h_bytes) *d2h_bytes = d2h;
   return DYPLAN_OK;
@@ -638,6 +698,7 @@ int dyplan_compile_linear_host(dyplan_ctx* ctx, const dyplan_batch* in, const fl
   dyplan_linear_extra dex;
   dex.dtau = (extra && extra->dtau) ? ar.take<int32_t>(hp.nrec) : nullptr;
   dex.quality = (extra && extra->quality) ? ar.take<double>(hp.nrec) : nullptr;
+  const char* stage = nullptr; const char* abase = nullptr;   // (this entry point copies array by array)
   if ((rc = dyplan_compile_linear(ctx, &d, dcost, params, L, levels, &dout, &dex, stream))) return rc;
   if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h))) return rc;
   if (dex.dtau) D2H(extra->dtau, dex.dtau, hp.nrec, int32_t);
@@ -677,6 +738,7 @@ int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bun
   int32_t* dvar = ar.take<int32_t>(hp.R);
   dyplan_bundle dres;
   if (rescored) bundle_alloc(ar, hp.R, hp.B, rescored->corr64 != nullptr, &dres);
+  const char* stage = nullptr; const char* abase = nullptr;   // (this entry point copies array by array)
   if ((rc = dyplan_select(ctx, &d, &dbundle, L, dlive, dvar, rescored ? &dres : nullptr, stream))) return rc;
   D2H(variant, dvar, hp.R, int32_t);
   if (rescored && (rc = bundle_to_host(ctx, &dres, rescored, hp.R, hp.B, s, d2h))) return rc;

@@ -21,6 +21,10 @@ constexpr uint64_t kNoIdx = ~0ull;
 constexpr int kClassWide = 0;        // int32 slack DP (k_score): any request the ABI admits
 constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): exact when every latency / demand sum is below 2^22, else a
                                      // conservative screen whose candidates are verified in int32 (ReqHdr.approx); tables <= kFastBlobWords
+constexpr int kClassSmall = 2;       // a small request of a small call: int32 layout, solved by k_small (dyplan_small.cu)
+constexpr int kSmallMaxR = 32;       // calls of at most this many requests try the small path
+constexpr int kSmallThreads = 128;
+constexpr unsigned long long kSmallMaxEvals = 1ull << 21;   // (plan, level) evaluations of a request k_small takes
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
 constexpr uint32_t kFastItemsPerWarp = 12;   // work items to aim for per resident warp (measured: 8 and 24 lose 4-7 % on cfg4)
@@ -98,6 +102,8 @@ struct CallState {
   uint32_t small_call_f;            // fast class: fewer than ~1K outer indices per resident warp (items are not lane-aligned)
   uint32_t tail_start_f;            // fast class: requests >= this index are cut into 4x smaller items (they are handed out last: a short tail)
   uint32_t approx_requests;         // fast class: requests verified in int32 (ReqHdr.approx)
+  uint32_t small_requests;          // requests solved by k_small
+  uint32_t pad0;
 };
 // outer indices per item of request r before rounding (k_plan and k_fscore must agree)
 __host__ __device__ inline unsigned long long fast_pif_of(unsigned long long pif, uint32_t tail_start, long long r) {
@@ -114,6 +120,8 @@ struct CallArgs {                   // passed by value to the kernels
   uint32_t flags;
   uint32_t ctx_flags;               // DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS (dyplan_set_flags)
   int32_t is_replan;
+  int32_t small_mode;               // R <= kSmallMaxR: requests of at most kSmallMaxEvals evaluations are staged for k_small
+  int32_t small_split;              // blocks per request in k_small (about 4 blocks per SM over the call)
   // scratch
   uint32_t* blob;                   // staged requests
   uint32_t* item_off;               // [R+1] wide class
@@ -131,6 +139,7 @@ struct CallArgs {                   // passed by value to the kernels
 cudaError_t launch_stage(const CallArgs& a, cudaStream_t s);
 cudaError_t launch_plan(const CallArgs& a, cudaStream_t s);
 cudaError_t launch_seed(const CallArgs& a, cudaStream_t s);
+cudaError_t launch_small(const CallArgs& a, cudaStream_t s);
 typedef cudaError_t (*score_launcher_t)(const CallArgs& a, int nb_class, int grid, cudaStream_t s);
 typedef cudaError_t (*fscore_launcher_t)(const CallArgs& a, int grid, cudaStream_t s);
 cudaError_t launch_score(const CallArgs& a, int grid, cudaStream_t s);

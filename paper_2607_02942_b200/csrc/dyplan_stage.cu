@@ -75,6 +75,11 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
 
   if (lane == 0) a.done[r] = 0;
   if (lane < L) a.gthr[r * L + lane] = 0.0f;
+  if (r == 0 && lane == 0) {   // (k_small adds to total_plans; k_plan, when it runs, sets every field)
+    CallState* st = a.st;
+    st->total_plans = 0; st->total_outer = 0; st->slow_steps = 0; st->bound_skipped = 0; st->total_items = 0; st->total_items_f = 0;
+    st->next_item = 0; st->next_item_f = 0; st->fast_requests = 0; st->approx_requests = 0; st->small_requests = 0;
+  }
 
   // ---- shape checks, in the oracle's order (load_req, validate, dispatched set, size of the free space) ----
   int st = DYPLAN_ST_OK;
@@ -209,7 +214,18 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   const int nbc = !has_caps ? 0 : (B <= 2 ? 2 : (B == 3 ? 3 : (B == 4 ? 4 : 8)));
   // the fp32 scorer is exact when every slack / demand sum is an integer below 2^23; beyond that its slacks are upper
   // bounds (directed rounding) and candidates are verified with int32 tables (ReqHdr.approx)
-  const bool fast_pre = min_c >= 1e-30;
+  // small call, small request: the int32 layout, solved by k_small without seeds, items or a persistent grid
+  bool small = false;
+  if (a.small_mode) {
+    unsigned long long pf = (e >= 0 && !fixed) ? (unsigned long long)myK : 1ull;   // <= 16^16: no overflow
+#pragma unroll
+    for (int off = 16; off; off >>= 1) {
+      const unsigned long long o = __shfl_xor_sync(0xffffffffu, pf, off);
+      pf = (pf > kSmallMaxEvals || o > kSmallMaxEvals) ? kSmallMaxEvals + 1 : pf * o;
+    }
+    small = pf * (unsigned long long)L <= kSmallMaxEvals;
+  }
+  const bool fast_pre = min_c >= 1e-30 && !small;
   const bool approx = !(sum_lat <= (1ll << 22) && (!has_caps || sum_dem <= (1ll << 22)));
   // options kept per node: all of them, or (opt-in, fast class only) the ones no other option dominates
   const uint32_t keep_full = (e >= 0 && !fixed) ? (myK >= 32 ? 0xffffffffu : ((1u << myK) - 1u)) : 1u;
@@ -295,7 +311,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     h->slo = b.slo_us[r]; h->nslots_pad = nslots_pad; h->n0 = n0; h->conn01 = (deps0 >> 1) & 1;
     h->skip_mask = residual ? fmask : 0u; h->outer_total = outer; h->base_idx = base;
     for (int bb = 0; bb < 8; bb++) h->cap[bb] = (b.cap && bb < B) ? b.cap[r * B + bb] : INT32_MAX;
-    h->klass = fast ? kClassFast : kClassWide; h->nbc = fast ? nbc : 0; h->Lp = Lp;
+    h->klass = fast ? kClassFast : (small ? kClassSmall : kClassWide); h->nbc = fast ? nbc : 0; h->Lp = Lp;
     const long long slo = b.slo_us[r];
     h->slo_f = __ll2float_ru(slo < sum_lat ? slo : sum_lat);
     h->slo_c = (int32_t)(slo < sum_lat ? slo : sum_lat);
@@ -512,20 +528,24 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   const long long chunk = (R + 1023) / 1024;
   const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
   unsigned long long so = 0, sf = 0, sp = 0, mxf = 0;
-  uint32_t nf = 0, na = 0;
+  uint32_t nf = 0, na = 0, ns = 0;
   __shared__ uint32_t s_na[1024];
+  __shared__ uint32_t s_ns;
   __shared__ unsigned long long s_mxf;
-  if (tid == 0) s_mxf = 0;
+  if (tid == 0) { s_mxf = 0; s_ns = 0; }
   __syncthreads();
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     if (h->status == DYPLAN_ST_OK) {
-      if (h->klass == kClassFast) { sf += h->outer_total; nf++; na += h->approx ? 1u : 0u; mxf = h->outer_total > mxf ? h->outer_total : mxf; } else so += h->outer_total;
+      if (h->klass == kClassFast) { sf += h->outer_total; nf++; na += h->approx ? 1u : 0u; mxf = h->outer_total > mxf ? h->outer_total : mxf; }
+      else if (h->klass == kClassWide) so += h->outer_total;
+      else ns++;
       sp += h->outer_total * (unsigned long long)(h->K0 * h->K1);
     }
   }
   s_sum[tid] = so; s_sumf[tid] = sf; s_plans[tid] = sp; s_nf[tid] = nf; s_na[tid] = na;
   if (mxf) atomicMax(&s_mxf, mxf);
+  if (ns) atomicAdd(&s_ns, ns);
   __syncthreads();
   for (int off = 512; off; off >>= 1) {
     if (tid < off) { s_sum[tid] += s_sum[tid + off]; s_sumf[tid] += s_sumf[tid + off]; s_plans[tid] += s_plans[tid + off]; s_nf[tid] += s_nf[tid + off]; s_na[tid] += s_na[tid + off]; }
@@ -565,7 +585,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   uint32_t cw = 0, cf = 0;
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
-    if (h->status != DYPLAN_ST_OK) continue;
+    if (h->status != DYPLAN_ST_OK || h->klass == kClassSmall) continue;
     if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_f); cf += (uint32_t)((h->outer_total + q - 1) / q); }
     else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
@@ -578,7 +598,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     a.item_off[r] = runw;
     a.item_off_f[r] = runf;
-    if (h->status != DYPLAN_ST_OK) continue;
+    if (h->status != DYPLAN_ST_OK || h->klass == kClassSmall) continue;
     if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_f); runf += (uint32_t)((h->outer_total + q - 1) / q); }
     else runw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
@@ -589,7 +609,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
     st->slow_steps = 0; st->bound_skipped = 0;
     st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
-    st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u; st->tail_start_f = tail_start; st->approx_requests = s_na[0];
+    st->fast_requests = n_fast; st->small_call_f = small_f ? 1u : 0u; st->tail_start_f = tail_start; st->approx_requests = s_na[0]; st->small_requests = s_ns; st->pad0 = 0;
   }
 }
 

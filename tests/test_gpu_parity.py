@@ -25,13 +25,35 @@ def dy():
     ctx.close()
 
 
+RECORD_KEYS = ("status", "plan_idx", "choice", "corr", "corr64", "lat", "dem", "dom_model")
+
+
 def gpu_run(dy, w, corr64=True):
+    """One call through the C ABI.  A call of at most 32 requests runs twice: as it stands (small requests take the
+    admission-path kernel k_small) and with DYPLAN_NO_SMALL_PATH (everything through the batched scorers); the two
+    must agree bit for bit, and the batched result is returned (dyplan_last_stats then describes that call)."""
     import torch
     binding, ctx = dy
     dw = binding.upload(w, "cuda:0", corr64)
     binding.launch(ctx, dw)
     torch.cuda.synchronize()
-    return dw.out.host()
+    g = dw.out.host()
+    if w.batch.R <= 32 and not (ctx.flags & binding.NO_SMALL_PATH):
+        f0 = ctx.flags
+        n_small = ctx.dyplan_last_stats()["small_requests"]
+        ctx.dyplan_set_flags(f0 | binding.NO_SMALL_PATH)
+        try:
+            dw2 = binding.upload(w, "cuda:0", corr64)
+            binding.launch(ctx, dw2)
+            torch.cuda.synchronize()
+            g2 = dw2.out.host()
+        finally:
+            ctx.dyplan_set_flags(f0)
+        for k in RECORD_KEYS:
+            if g[k] is not None:
+                assert np.array_equal(g[k], g2[k]), f"{w.name}: {k} differs between the small path ({n_small} requests) and the batched scorers"
+        return g2
+    return g
 
 
 def both(dy, orc, w, where):
@@ -185,6 +207,58 @@ def test_duplicate_options_exact_ties(dy, orc):
     b.acc[:] = np.round(b.acc * 8) / 8          # few distinct accuracies -> many exact C ties
     b.vuln[:] = np.round(b.vuln * 4) / 4
     g, ref, c = both(dy, orc, w, "ties")
+
+
+# ---- the admission path: small calls (k_small) ------------------------------------------------------------------------
+def test_small_call_path_takes_small_requests_only(dy, orc):
+    import torch
+    binding, ctx = dy
+    # configs[0] alone: one launch pair (stage + small) through the host entry point, six through the device one
+    w = wl.make_config(0)
+    dw = binding.upload(w)
+    binding.launch(ctx, dw)
+    torch.cuda.synchronize()
+    st = ctx.dyplan_last_stats()
+    assert st["small_requests"] == 1 and st["fast_requests"] == 0 and st["plans"] == w.n_plans_total() and st["launches"] == 6
+    check_records(orc, w, dw.out.host(), orc.run(w), where="small cfg0")
+    g, _, _ = binding.run_host(ctx, w)
+    st = ctx.dyplan_last_stats()
+    assert st["launches"] == 2 and st["small_requests"] == 1 and st["plans"] == w.n_plans_total()
+    check_records(orc, w, g, orc.run(w), where="small cfg0 host")
+    # a call that mixes one large request (8^8 x 4 evaluations: batched scorers) with small ones
+    big = wl.make_config(1, R=1)
+    small = wl.random_workload(301, R=5, nmin=1, nmax=5, kmin=1, kmax=6, B=2, M=2, L=4, caps=False)
+    b1, b2 = big.batch, small.batch
+    cat = lambda x, y: np.concatenate([x, y])
+    batch = wl.Batch(R=6, B=2, M=2, node_off=cat(b2.node_off, b2.node_off[-1] + b1.node_off[1:]).astype(np.int32),
+                     opt_off=cat(b2.opt_off, b2.opt_off[-1] + b1.opt_off[1:]).astype(np.int32),
+                     pred_mask=cat(b2.pred_mask, b1.pred_mask), vuln=cat(b2.vuln, b1.vuln), lat_us=cat(b2.lat_us, b1.lat_us),
+                     acc=cat(b2.acc, b1.acc), demand=cat(b2.demand, b1.demand), backend=cat(b2.backend, b1.backend),
+                     model=cat(b2.model, b1.model), slo_us=cat(b2.slo_us, b1.slo_us), cap=None)
+    reqs = wl.Workload(name="mixed-small", kind="compile", batch=batch, L=4, mult_pm=big.mult_pm.copy())
+    dw = binding.upload(reqs)
+    binding.launch(ctx, dw)
+    torch.cuda.synchronize()
+    st = ctx.dyplan_last_stats()
+    assert st["small_requests"] == 5 and st["fast_requests"] == 1 and st["plans"] == reqs.n_plans_total()
+    check_records(orc, reqs, dw.out.host(), orc.run(reqs), where="mixed small + large")
+    g, _, _ = binding.run_host(ctx, reqs)
+    assert ctx.dyplan_last_stats()["launches"] == 6           # not all small: the batched scorers run too
+    check_records(orc, reqs, g, orc.run(reqs), where="mixed small + large, host")
+
+
+@pytest.mark.parametrize("seed,L,B,caps", [(311, 1, 1, False), (312, 3, 2, True), (313, 8, 3, True), (314, 4, 8, True)])
+def test_small_call_path_ragged(dy, orc, seed, L, B, caps):
+    # everything k_small must get right on its own: ragged N and K, tool nodes, caps with up to 8 backends, invalid and
+    # infeasible requests, replans in both modes (the helper compares with the batched scorers, then with the oracle)
+    w = wl.random_workload(seed, R=30, nmin=1, nmax=6, kmin=1, kmax=7, B=B, M=3, L=L, caps=caps)
+    w.batch.slo_us[3] = 0                      # infeasible
+    w.batch.vuln[int(w.batch.node_off[5])] = np.nan     # invalid
+    g = gpu_run(dy, w)
+    check_records(orc, w, g, orc.run(w), where=f"small-ragged(seed={seed})")
+    for flags in (wl.FLAG_FIXED_IN_PLACE, wl.FLAG_RESIDUAL):
+        wr = wl.random_replan_workload(seed + 50, R=28, nmin=1, nmax=7, kmin=1, kmax=6, B=B, M=3, caps=caps, flags=flags)
+        check_records(orc, wr, gpu_run(dy, wr), orc.run(wr), where=f"small-replan(seed={seed})")
 
 
 # ---- scorer classes: fp32 slack DP for small exact ranges, int32 slack DP for the rest ----------------
@@ -641,7 +715,7 @@ def test_bounds_and_dominance_pruning_together(dy, orc):
             w = wl.random_workload(seed, R=40, nmin=1, nmax=7, kmin=1, kmax=8, B=B, M=3, L=L, caps=caps)
             check_records(orc, w, gpu_run(dy, w), orc.run(w), where=f"bounded+pruned(seed={seed})")
         with pytest.raises(binding.DyplanError) as e:
-            ctx.dyplan_set_flags(4)                              # unknown bit
+            ctx.dyplan_set_flags(1 << 10)                        # unknown bit
         assert e.value.code == binding.ERR_ARG
     finally:
         ctx.dyplan_set_flags(0)
