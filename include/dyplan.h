@@ -22,7 +22,9 @@
  *   The caller owns every buffer and keeps it alive until the stream work completes.  The library allocates only
  *   its own scratch inside dyplan_ctx (grown on demand; growing calls cudaMalloc, nothing else synchronises).
  * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Plain calls are
- *   asynchronous on it.  A ctx is not thread-safe; separate ctxs are independent.
+ *   asynchronous on it.  A ctx owns one set of scratch: a call issued on another stream than the previous call of the
+ *   same ctx first waits, on the device, for that call's work (an event; the host does not block), so calls of one ctx
+ *   never overlap -- use one ctx per stream for concurrency.  A ctx is not thread-safe; separate ctxs are independent.
  * Errors: every call returns 0 or a negative DYPLAN_ERR_* code; nothing throws, aborts or prints.  Problems
  *   only a device can see (malformed DAG, out-of-range table entries, NaN, overflow, plan space too large,
  *   dispatched set not predecessor-closed) are reported per request in dyplan_bundle.status; the other requests

@@ -11,7 +11,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "linear_oracle.c")
-_OUT = os.path.join(_HERE, "_build", "liblinorc.so")
+# ORACLE_SANITIZE=1 builds a separate library with AddressSanitizer + UndefinedBehaviorSanitizer (the test process must
+# then run with LD_PRELOAD=$(gcc -print-file-name=libasan.so); see profiles/r2_sanitizers.md).  Build plumbing only.
+_SAN = bool(os.environ.get("ORACLE_SANITIZE"))
+_OUT = os.path.join(_HERE, "_build", "liblinorc_san.so" if _SAN else "liblinorc.so")
 _lock = threading.Lock()
 _lib = None
 
@@ -22,7 +25,8 @@ def build(force: bool = False) -> str:
     os.makedirs(os.path.dirname(_OUT), exist_ok=True)
     if force or not os.path.exists(_OUT) or os.path.getmtime(_OUT) < os.path.getmtime(_SRC):
         tmp = _OUT + f".{os.getpid()}.tmp"
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra",
+        san = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"] if _SAN else []
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra", *san,
                                "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _OUT)
     return _OUT

@@ -76,6 +76,9 @@ struct dyplan_ctx {
   // last call
   cudaStream_t last_stream = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  cudaEvent_t ev_done = nullptr;   // end of the last call that used the ctx's scratch (ordering across streams)
+  cudaStream_t done_stream = nullptr;
+  bool have_done = false;
   bool have_events = false;
   int last_launches = 0;
   int last_L = 0;
@@ -99,6 +102,18 @@ static int ensure(dyplan_ctx* ctx, DevBuf& b, size_t bytes) {
   size_t want = bytes + bytes / 4 + 256;
   CK(cudaMalloc(&b.p, want));
   b.cap = want;
+  return DYPLAN_OK;
+}
+
+// The ctx owns ONE set of scratch (staged blobs, counters, partial records, the *_host arena).  Calls on one stream are
+// ordered by the stream; a call arriving on ANOTHER stream first waits (on the device) for the previous call's work.
+static int order_after_previous(dyplan_ctx* ctx, cudaStream_t stream) {
+  if (ctx->have_done && ctx->done_stream != stream) CK(cudaStreamWaitEvent(stream, ctx->ev_done, 0));
+  return DYPLAN_OK;
+}
+static int mark_done(dyplan_ctx* ctx, cudaStream_t stream) {
+  CK(cudaEventRecord(ctx->ev_done, stream));
+  ctx->done_stream = stream; ctx->have_done = true;
   return DYPLAN_OK;
 }
 
@@ -131,7 +146,8 @@ int dyplan_create(dyplan_ctx** out, int device_ordinal) {
   ctx->device = device_ordinal;
   if (cudaSetDevice(device_ordinal) != cudaSuccess ||
       cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device_ordinal) != cudaSuccess ||
-      cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
+      cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_done, cudaEventDisableTiming) != cudaSuccess) {
     delete ctx;
     return DYPLAN_ERR_CUDA;
   }
@@ -156,6 +172,7 @@ int dyplan_destroy(dyplan_ctx* ctx) {
   if (ctx->hstage) cudaFreeHost(ctx->hstage);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+  if (ctx->ev_done) cudaEventDestroy(ctx->ev_done);
   delete ctx;
   return DYPLAN_OK;
 }
@@ -204,6 +221,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   if (rc) return rc;
   CK(cudaSetDevice(ctx->device));
 
+  if ((rc = order_after_previous(ctx, stream))) return rc;
   const size_t R = (size_t)in->R;
   const int nbc = nb_class_of(in->B, in->cap != nullptr);
   int& occ = ctx->occ[L - 1][nb_index(nbc)];
@@ -242,12 +260,12 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   CK(launch_stage(a, stream));
   int launches = 1;
   const bool only_small = a.small_mode && all_small;
-  if (only_small) CK(cudaEventRecord(ctx->ev0, stream));   // (score_ms: k_small here, else the batched scorers)
-  if (a.small_mode) { CK(launch_small(a, stream)); launches++; }   // small requests of a small call: solved here (admission path)
+  // score_ms brackets the scorers: from k_small on in a small call, else the two batched scorers
+  if (a.small_mode) { CK(cudaEventRecord(ctx->ev0, stream)); CK(launch_small(a, stream)); launches++; }   // admission path
   if (!only_small) {
     CK(launch_seed(a, stream));
     CK(launch_plan(a, stream));
-    CK(cudaEventRecord(ctx->ev0, stream));
+    if (!a.small_mode) CK(cudaEventRecord(ctx->ev0, stream));
     CK(kFLaunch[L - 1](a, fgrid, stream));      // fp32 scorer: requests of the fast class
     CK(kLaunch[L - 1](a, nbc, grid, stream));   // int32 scorer: the rest (exits at once when it has no work items)
     launches += 4;
@@ -255,7 +273,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   CK(cudaEventRecord(ctx->ev1, stream));
   ctx->have_events = true;
   ctx->last_launches = launches;
-  return DYPLAN_OK;
+  return mark_done(ctx, stream);
 }
 
 extern "C" {
@@ -365,6 +383,7 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   if (params->effort > 1.0f) return DYPLAN_ERR_ARG;
   for (int l = 0; l < L; l++) if (!(levels[l] >= 0.0f) || levels[l] > 1e6f) return DYPLAN_ERR_ARG;
   CK(cudaSetDevice(ctx->device));
+  if ((rc = order_after_previous(ctx, s))) return rc;
   const size_t R = (size_t)in->R;
   if ((rc = ensure(ctx, ctx->lin_blob, R * kLinBlobWords * 4))) return rc;
   if ((rc = ensure(ctx, ctx->lin_misc, 64))) return rc;
@@ -388,7 +407,7 @@ int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, const float* 
   CK(cudaEventRecord(ctx->ev1, s));
   ctx->have_events = true;
   ctx->last_launches = 3;
-  return DYPLAN_OK;
+  return mark_done(ctx, s);
 }
 
 int dyplan_measure_issue_rates(dyplan_ctx* ctx, dyplan_issue_rate* out, int32_t capacity, int32_t* n_out, float* sm_clock_mhz,

@@ -556,6 +556,25 @@ def test_switch_parity(dy, orc, seed):
     assert e.value.code == binding.ERR_ARG
 
 
+def test_calls_on_different_streams_of_one_ctx_are_ordered(dy, orc):
+    # a ctx has one set of scratch: a call on another stream waits (on the device) for the previous call of the ctx
+    import torch
+    binding, ctx = dy
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    w1 = wl.make_config(2, R=96)
+    w2 = wl.random_workload(88, R=40, nmin=2, nmax=7, kmin=1, kmax=6, B=2, M=3, L=3, caps=True)
+    d1, d2 = binding.upload(w1), binding.upload(w2)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        binding.launch(ctx, d1, s1)
+        binding.launch(ctx, d2, s2)        # would reset the counters the first call's scorers are pulling from
+    torch.cuda.synchronize()
+    check_records(orc, w2, d2.out.host(), orc.run(w2), where="two streams, second call")
+    ref1 = orc.run(w1, 0, 12)
+    g1 = d1.out.host()
+    check_records(orc, w1, g1, ref1, records=range(12 * w1.L), where="two streams, first call")
+
+
 def test_api_argument_errors(dy):
     binding, ctx = dy
     w = wl.random_workload(81, R=2, nmin=2, nmax=3, kmin=2, kmax=3, B=2, M=2, L=2, caps=False)
