@@ -147,7 +147,18 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
   // one of THIS lane's plans ties or beats it
   for (int l = 0; l < LT; l++) { best[l] = l < L ? dec_f32(__ldcg(&a.gJ[r * L + l])) : INFINITY; kmin[l] = ~0ull; }
 
-  float u[16];
+  // outer nodes (>= 3): odometer over their digits; a step recomputes the slack DP, the weight / duration prefix sums and
+  // the canonical index from the highest digit that changed down to node 3 (one node on average), instead of decoding
+  // the outer index by div / mod and redoing every node
+  float u[16], Wa[17], Da[17], Ra[17];
+  unsigned long long Ia[17];
+  int dig[16];
+  Wa[Np] = 0.0f; Da[Np] = 0.0f; Ra[Np] = 0.0f; Ia[Np] = 0ull;
+  {
+    unsigned long long t = ob < oe ? ob : 0ull;
+    for (int i = 3; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; }
+  }
+  int top = Np - 1;
   for (unsigned long long step = 0; step < lper; step++) {   // the same trip count on every lane: the loop shuffles
     // share the climb: every lane's incumbent rises to the best J any lane of the warp has reached (a lane whose
     // incumbent is raised by another lane's plan no longer holds a plan attaining it: its key is cleared)
@@ -160,18 +171,25 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
     }
     const unsigned long long o = ob + step;
     if (o >= oe) continue;
-    unsigned long long t = o, idxo = 0;
-    int dig[16];
-    for (int i = 3; i < Np; i++) { const unsigned long long k = (unsigned long long)h->K[i]; dig[i] = (int)(t % k); t /= k; idxo += (unsigned long long)dig[i] * h->stride[i]; }
-    float Wp = 0.0f, Dp = 0.0f, Rm = 0.0f;
-    for (int i = Np - 1; i >= 3; --i) {
+    for (int i = top; i >= 3; --i) {
       const float2 wd = t_wd[h->optbase[i] + dig[i]];
       float m = 0.0f;
       for (uint32_t dm = h->succ[i]; dm; dm &= dm - 1) m = fminf(m, u[__ffs(dm) - 1]);
       u[i] = m - wd.y;
-      Rm = fminf(Rm, u[i]);
-      Wp += wd.x;
-      Dp += wd.y;
+      Ra[i] = fminf(Ra[i + 1], u[i]);
+      Wa[i] = Wa[i + 1] + wd.x;
+      Da[i] = Da[i + 1] + wd.y;
+      Ia[i] = Ia[i + 1] + (unsigned long long)dig[i] * h->stride[i];
+    }
+    const float Wp = Wa[3], Dp = Da[3], Rm = Ra[3];
+    const unsigned long long idxo = Ia[3];
+    {   // advance the odometer for the next step
+      int i = 3;
+      for (; i < Np; i++) {
+        if (++dig[i] < h->K[i]) break;
+        dig[i] = 0;
+      }
+      top = i < Np ? i : Np - 1;
     }
     float u2in = 0.0f, u1in3 = 0.0f, a0in3 = 0.0f;
     for (uint32_t dm = succ2; dm; dm &= dm - 1) u2in = fminf(u2in, u[__ffs(dm) - 1]);
