@@ -305,6 +305,26 @@ typedef struct {
 DYPLAN_API int dyplan_measure_issue_rates(dyplan_ctx* ctx, dyplan_issue_rate* out, int32_t capacity, int32_t* n_out,
                                float* sm_clock_mhz, void* stream);
 
+/* dyplan_compile for callers that must not allocate device memory (work under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same kernels, the same records, but every byte of scratch (staged request
+ * blobs, work-item offsets, tickets, incumbent thresholds, partial records, call state) is carved from ONE file-scope
+ * `static __device__` array of DYPLAN_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library
+ * holds until the process exits.  The call allocates nothing: no cudaMalloc / cudaFree / cudaMallocHost, no growth of
+ * the ctx's own scratch (which it does not touch), no host heap.  `in`, `mult_pm`, `out`: DEVICE pointers, exactly as
+ * in dyplan_compile; the caller owns inputs and outputs.  Asynchronous on `stream`.
+ * Limits: 1 <= L <= 8 as everywhere, and R <= DYPLAN_STATIC_MAX_REQUESTS; a larger R returns DYPLAN_ERR_STATIC_LIMIT
+ * (nothing is launched, dyplan_last_cuda_error() holds a sentence naming R and the limit).
+ * Sharing: the array is ONE per device for the whole process -- every ctx and every call of this entry point uses it,
+ * and it keeps the previous call's contents (the kernels reset the counters they need at the start of each call, as
+ * they do for the ctx's scratch).  Two calls that OVERLAP on the GPU (different streams, different ctxs, different
+ * host threads) RACE on it and give garbage: issue them on one stream, or order them with events.  The library adds no
+ * ordering of its own here.  dyplan_last_stats after this call reports `launches` and `sm_count` only. */
+#define DYPLAN_STATIC_MAX_REQUESTS 512
+#define DYPLAN_STATIC_SCRATCH_BYTES (16u << 20)
+#define DYPLAN_ERR_STATIC_LIMIT (-5) /* the call does not fit the static scratch of dyplan_compile_static */
+DYPLAN_API int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
+                          void* stream);
+
 DYPLAN_API const char* dyplan_strerror(int code);
 DYPLAN_API const char* dyplan_last_cuda_error(const dyplan_ctx* ctx); /* "" if none */
 DYPLAN_API int dyplan_version(void);                            /* major*10000 + minor*100 + patch */

@@ -21,7 +21,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdyplan.so")
 
 ST_OK, ST_INFEASIBLE, ST_INVALID, ST_TOO_LARGE = 0, 1, 2, 3
-ERR_NULL, ERR_LIMIT, ERR_CUDA, ERR_ARG = -1, -2, -3, -4
+ERR_NULL, ERR_LIMIT, ERR_CUDA, ERR_ARG, ERR_STATIC_LIMIT = -1, -2, -3, -4, -5
+STATIC_MAX_REQUESTS = 512          # DYPLAN_STATIC_MAX_REQUESTS
+STATIC_SCRATCH_BYTES = 16 << 20    # DYPLAN_STATIC_SCRATCH_BYTES
 FIXED_IN_PLACE, RESIDUAL = 0, 1
 NO_IDX = np.iinfo(np.uint64).max
 
@@ -29,6 +31,7 @@ EXPORTS = (
     "dyplan_create", "dyplan_destroy", "dyplan_set_flags", "dyplan_compile", "dyplan_replan", "dyplan_select", "dyplan_switch", "dyplan_compile_linear", "dyplan_compile_linear_host", "dyplan_bind",
     "dyplan_compile_host", "dyplan_replan_host", "dyplan_select_host", "dyplan_last_stats",
     "dyplan_strerror", "dyplan_last_cuda_error", "dyplan_version", "dyplan_measure_issue_rates",
+    "dyplan_compile_static",
 )
 
 
@@ -102,6 +105,7 @@ def lib():
         l.dyplan_set_flags.argtypes = [vp, u32]
         l.dyplan_compile.argtypes = [vp, pb, i32, vp, po, vp]
         l.dyplan_replan.argtypes = [vp, pb, vp, vp, vp, u32, po, vp]
+        l.dyplan_compile_static.argtypes = [vp, pb, i32, vp, po, vp]
         l.dyplan_select.argtypes = [vp, pb, po, i32, vp, vp, po, vp]
         l.dyplan_compile_linear.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp]
         l.dyplan_compile_linear_host.argtypes = [vp, pb, vp, C.POINTER(CLinearParams), i32, vp, po, C.POINTER(CLinearExtra), vp, pu64, pu64]
@@ -273,13 +277,18 @@ class Context:
     def _check(self, rc: int):
         if rc:
             msg = dyplan_strerror(rc)
-            if rc == ERR_CUDA:
+            if rc in (ERR_CUDA, ERR_STATIC_LIMIT):
                 msg += ": " + lib().dyplan_last_cuda_error(self._h).decode()
             raise DyplanError(rc, msg)
 
     def dyplan_compile(self, batch: Buffers, L: int, mult_pm, out: Buffers, stream=None):
         self._check(lib().dyplan_compile(self._h, C.byref(batch.cstruct), L, _ptr(mult_pm), C.byref(out.cstruct),
                                          _stream_ptr(stream)))
+
+    def dyplan_compile_static(self, batch: Buffers, L: int, mult_pm, out: Buffers, stream=None):
+        """dyplan_compile with every byte of scratch in the library's static device array: no allocation."""
+        self._check(lib().dyplan_compile_static(self._h, C.byref(batch.cstruct), L, _ptr(mult_pm),
+                                                C.byref(out.cstruct), _stream_ptr(stream)))
 
     def dyplan_replan(self, batch: Buffers, dispatched_mask, fixed_choice, live_mult_pm, flags: int, out: Buffers,
                       stream=None):

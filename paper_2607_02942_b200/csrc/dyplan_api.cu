@@ -3,6 +3,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include "dyplan_internal.cuh"
@@ -130,6 +131,7 @@ const char* dyplan_strerror(int code) {
     case DYPLAN_ERR_LIMIT: return "R, B, M, L, NN or KK outside the supported limits";
     case DYPLAN_ERR_CUDA: return "a CUDA runtime call failed (see dyplan_last_cuda_error)";
     case DYPLAN_ERR_ARG: return "invalid argument";
+    case DYPLAN_ERR_STATIC_LIMIT: return "the call exceeds the static scratch of dyplan_compile_static (R > DYPLAN_STATIC_MAX_REQUESTS = 512)";
     default: return "unknown error";
   }
 }
@@ -768,3 +770,124 @@ int dyplan_select_host(dyplan_ctx* ctx, const dyplan_batch* in, const dyplan_bun
 }
 
 }  // extern "C"
+
+// ---- dyplan_compile_static: the compile call with no device allocation (include/dyplan.h) -------------------------
+// The scorers' scratch normally lives in buffers the ctx grows with cudaMalloc.  Here it is carved from one file-scope
+// device array, so the call is usable where cudaMalloc is not (graph capture, serving loops).  The array is shared by
+// every ctx and call on a device and keeps the last call's contents: k_stage / k_plan reset the tickets, thresholds and
+// counters at the start of every call, exactly as they do for the ctx's own (equally unzeroed, reused) buffers.
+static __device__ __align__(256) unsigned char g_static_scratch[DYPLAN_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// In host code `g_static_scratch` is only the host-side shadow of the symbol, not a device address: the address the
+// kernels can use is looked up once per device, with that device current, and cached.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned char* g_static_ptr[kStaticMaxDevices];   // zero-initialised: not looked up yet
+
+cudaError_t static_scratch_base(int device, unsigned char** base) {
+  if (device < 0 || device >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);   // the caller made `device` current
+    if (e != cudaSuccess) return e;
+    if (!p || ((uintptr_t)p & 255u)) return cudaErrorInvalidSymbol;
+    g_static_ptr[device] = (unsigned char*)p;
+  }
+  *base = g_static_ptr[device];
+  return cudaSuccess;
+}
+
+struct StaticCarver {   // 256-byte aligned pieces of the array; `off` is what the layout needs in total
+  unsigned char* base;
+  size_t off = 0;
+  template <typename T>
+  T* take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = (T*)(base + off);
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+// work-item budget of a static call: 2R+2 records of rounding slack plus 32768 items per scorer class (k_plan cuts
+// coarser items when a class would need more, so any plan space still fits)
+constexpr uint32_t kStaticItemsPerClass = 32768;
+
+}  // namespace
+
+extern "C" int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
+                                     void* stream_) {
+  if (!ctx) return DYPLAN_ERR_NULL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  int rc = check_batch(in, true);
+  if (rc) return rc;
+  if (L < 1 || L > DYPLAN_MAX_LEVELS) return DYPLAN_ERR_LIMIT;
+  ctx->last_launches = 0;
+  ctx->have_events = false;   // (dyplan_last_stats: launches and sm_count only)
+  ctx->last_stream = stream;
+  ctx->last_L = L;
+  ctx->last_linear = false;
+  if (in->R == 0) return DYPLAN_OK;
+  if (!mult_pm) return DYPLAN_ERR_NULL;
+  if ((rc = check_bundle(out))) return rc;
+  if (in->R > DYPLAN_STATIC_MAX_REQUESTS) {
+    snprintf(ctx->errbuf, sizeof(ctx->errbuf), "dyplan_compile_static: R = %d requests exceed DYPLAN_STATIC_MAX_REQUESTS = %d "
+             "(static scratch of %u bytes); use dyplan_compile", (int)in->R, DYPLAN_STATIC_MAX_REQUESTS, (unsigned)DYPLAN_STATIC_SCRATCH_BYTES);
+    return DYPLAN_ERR_STATIC_LIMIT;
+  }
+  CK(cudaSetDevice(ctx->device));
+  unsigned char* base = nullptr;
+  CK(static_scratch_base(ctx->device, &base));
+
+  const size_t R = (size_t)in->R;
+  const int nbc = nb_class_of(in->B, in->cap != nullptr);
+  int& occ = ctx->occ[L - 1][nb_index(nbc)];
+  if (occ <= 0) {
+    occ = kOcc[L - 1](nbc);
+    if (occ <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
+  }
+  int& focc = ctx->focc[L - 1];
+  if (focc <= 0) {
+    focc = kFOcc[L - 1]();
+    if (focc <= 0) return fail_cuda(ctx, cudaGetLastError() == cudaSuccess ? cudaErrorLaunchOutOfResources : cudaPeekAtLastError());
+  }
+  const int grid = ctx->sm_count * occ;
+  const int fgrid = ctx->sm_count * focc;
+  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * kFastItemsPerWarp;
+  const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * kStaticItemsPerClass;
+
+  CallArgs a;
+  memset(&a, 0, sizeof(a));
+  a.in = *in; a.out = *out; a.L = L; a.mult = mult_pm; a.ctx_flags = ctx->flags;
+  a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
+  a.small_split = a.small_mode ? (4 * ctx->sm_count / (int)in->R > 1 ? 4 * ctx->sm_count / (int)in->R : 1) : 1;
+  StaticCarver sc{base};
+  a.blob = sc.take<uint32_t>(R * blob_stride_words(L));
+  a.item_off = sc.take<uint32_t>(2 * (R + 1)); a.item_off_f = a.item_off + (R + 1);
+  a.done = sc.take<uint32_t>(R);
+  a.gthr = sc.take<float>(R * L);
+  // k_small writes small_split records per request, the batched scorers one per work item: room for the larger
+  const size_t small_recs = a.small_mode ? R * (size_t)a.small_split : 0;
+  a.partial = sc.take<Partial>((small_recs > max_items ? small_recs : (size_t)max_items) * L);
+  a.st = sc.take<CallState>(1);
+  a.target_items_f = target_items_f;
+  a.max_items = max_items;
+  if (sc.off > (size_t)DYPLAN_STATIC_SCRATCH_BYTES) {   // (cannot happen within the limits above: a guard for a device with > 1000 SMs)
+    snprintf(ctx->errbuf, sizeof(ctx->errbuf), "dyplan_compile_static: the scratch layout needs %zu bytes, the static array holds %u",
+             sc.off, (unsigned)DYPLAN_STATIC_SCRATCH_BYTES);
+    return DYPLAN_ERR_STATIC_LIMIT;
+  }
+
+  CK(launch_stage(a, stream));
+  int launches = 1;
+  if (a.small_mode) { CK(launch_small(a, stream)); launches++; }
+  CK(launch_seed(a, stream));
+  CK(launch_plan(a, stream));
+  CK(kFLaunch[L - 1](a, fgrid, stream));
+  CK(kLaunch[L - 1](a, nbc, grid, stream));
+  ctx->last_launches = launches + 4;
+  return DYPLAN_OK;
+}

@@ -33,7 +33,8 @@ def test_header_declares_the_three_calls():
     assert "dyplan_bind" in names
     assert "dyplan_set_flags" in names
     assert "dyplan_measure_issue_rates" in names
-    assert len(names) == 18
+    assert "dyplan_compile_static" in names
+    assert len(names) == 19
 
 
 def test_library_exports_every_declared_symbol(binding):
