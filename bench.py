@@ -5,7 +5,8 @@ A "step" is one pass of the whole hot path (K_stage -> K_seed -> K_plan -> K_fsc
 reduce and bundle emission) over one batch of synthetic requests.  With no flags the run covers ALL FIVE configurations
 of BASELINE.json in one process (`"configs": [...]` in the JSON line, one entry each: Geval/s, plans/s, requests/s,
 ms_per_step, kernel_ms, roofline, e2e through the *_host C-ABI call, cpu_baseline = the oracle on a bounded sample),
-plus a wide-class line (configs[1] with latencies x 3000: requests beyond the fp32 scorer's plain range) and the
+plus a wide-class line (configs[1] with latencies x 3000: requests beyond the fp32 scorer's plain range), an int32-scorer
+line (configs[1] with one zero-factor option per request: the requests only k_score takes) and the
 variant selector (selects/s after configs[1], [2], [4]).  The headline `value` / `ms_per_step` / `config.workload` are
 those of the largest single-GPU configuration, configs[4] (2.79e11 (plan, level) evaluations per step).  Requests are
 independent, so with N > 1 every rank compiles its own batch of the same shape (different seed) and no data-path
@@ -140,12 +141,21 @@ class ClockSampler:
                 "reasons": [n for n, bit in self.REASONS if mask & bit]}
 
 
-def make_workload(cfg: int, rank: int, requests: int | None, wide: bool = False):
+def make_workload(cfg: int, rank: int, requests: int | None, wide=False):
     from support import workloads as wl
     # rank 0 runs the config's own seed; other ranks an independent batch of the same shape
     from paper_2607_02942_b200.multi import rank_seed
     w = wl.make_config(cfg, R=requests, seed=rank_seed(cfg, rank))
-    if wide:
+    if wide == "int32":
+        # one zero-factor option per request (v = 1, a = 0: that option gives C = 0): the fp32 screen needs C32 > 0 for
+        # real plans, so k_stage routes every such request to the int32 scorer k_score
+        b = w.batch
+        for r in range(b.R):
+            n = int(b.node_off[r]) + (r % b.n_nodes(r))
+            b.vuln[n] = 1.0
+            b.acc[int(b.opt_off[n])] = 0.0
+        w.name = w.name + " with one zero-factor option per request"
+    elif wide:
         # the paper's own latencies are seconds to minutes per request (Fig. 2: 4.2 s ... 414.5 s): scale
         # every duration and the SLO so that the requests leave the fp32 scorer's plain exact-integer range
         w.batch.lat_us = (w.batch.lat_us.astype(np.int64) * WIDE_FACTOR).astype(np.int32)
@@ -154,11 +164,13 @@ def make_workload(cfg: int, rank: int, requests: int | None, wide: bool = False)
     return w
 
 
-def workload_tag(cfg: int, wide: bool) -> str:
-    return f"cfg{cfg}" + ("_wide" if wide else "")
+def workload_tag(cfg: int, wide) -> str:
+    return f"cfg{cfg}" + ("_int32" if wide == "int32" else "_wide" if wide else "")
 
 
-def workload_label(cfg: int, wide: bool) -> str:
+def workload_label(cfg: int, wide) -> str:
+    if wide == "int32":
+        return f"BASELINE.json configs[{cfg}] with one zero-factor option per request (int32 scorer k_score)"
     return f"BASELINE.json configs[{cfg}]" + (f" with latencies x {WIDE_FACTOR} (seconds, PAPER.md:68)" if wide else "")
 
 
@@ -435,6 +447,7 @@ def run_dyplan(args, rank: int, world: int, local_rank: int):
     legs = [(c, False) for c in args.cfg_list]
     if args.wide and not prune_flags:
         legs.append((1, True))
+        legs.append((1, "int32"))
     entries, selects = [], []
     for cfg, wide in legs:
         entry, w, dw = bench_one(args, ctx, binding, torch, dist, dev, rank, world, cfg, wide, peaks, sampler, flush, stream, prune_flags)
@@ -623,7 +636,7 @@ def main():
     ap.add_argument("--impl", default="dyplan", choices=["dyplan", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-select", action="store_true")
-    ap.add_argument("--no-wide", dest="wide", action="store_false", help="skip the configs[1] x 3000-latency leg")
+    ap.add_argument("--no-wide", dest="wide", action="store_false", help="skip the configs[1] x 3000-latency leg and the int32-scorer leg")
     ap.add_argument("--objective", default="product", choices=["product", "linear"],
                     help="product: north_star's constrained objective (default); linear: the paper's Eq.(4)/(5)")
     ap.add_argument("--prune", default="none", choices=["none", "dominated", "bounds", "both"],

@@ -7,7 +7,7 @@
 //             incumbent per level -- best J32 and, among the plans attaining it, min (T << 40 | idx) -- in registers; the
 //             unrolled inner block only tests J >= incumbent and a group that has a hit is walked again to update.  The
 //             item's record per level = max J over the lanes, min key among the lanes attaining it (shuffles).
-//   k_lemit   one thread per (request, level): reduce the request's item records (J desc, key asc), decode the winner,
+//   k_lemit   one warp per (request, level): reduce the request's item records (J desc, key asc), decode the winner,
 //             annotate, re-evaluate J in fp64
 // J32 is a pure function of the plan: W is summed from the last node down, then one FFMA per term.
 #include "dyplan_common.cuh"
@@ -302,13 +302,16 @@ __global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
   }
 }
 
-// One thread per (request, level): decode the winner, annotate, re-evaluate J in fp64 (definition order of the oracle:
+// One warp per (request, level); lane 0 does the rest: decode the winner, annotate, re-evaluate J in fp64 (definition order of the oracle:
 // W summed in node order, then - lambda_l T - lambda_ld L D_tau; no contraction).
 __global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
-  const long long rec = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  // one WARP per record: a request with few peers is cut into thousands of items (a.chunks = 4736 for 6 requests), and
+  // one thread walking them serially took 0.5 ms; the lanes stride over the item records and reduce by shuffle
+  const long long rec = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   const dyplan_batch& b = a.in;
   const int L = a.L, B = b.B, M = b.M;
-  if (rec >= (long long)b.R * L) return;
+  if (rec >= (long long)b.R * L) return;   // warp-uniform
   const long long r = rec / L;
   const int l = (int)(rec % L);
   const LinHdr* h = (const LinHdr*)(a.blob + (size_t)r * kLinBlobWords);
@@ -316,11 +319,18 @@ __global__ void __launch_bounds__(128) k_lemit(LinArgs a) {
   const dyplan_bundle& o = a.out;
   float bestJ = -INFINITY;
   unsigned long long key = ~0ull;
-  for (uint32_t c = 0; c < a.chunks; c++) {
+  for (uint32_t c = lane; c < a.chunks; c += 32) {
     const LinRec rc = a.rec[((size_t)r * a.chunks + c) * L + l];
     if (rc.key == ~0ull) continue;                         // an item whose range was empty
     if (rc.J > bestJ || (rc.J == bestJ && rc.key < key)) { bestJ = rc.J; key = rc.key; }
   }
+#pragma unroll
+  for (int off = 16; off; off >>= 1) {
+    const float oJ = __shfl_xor_sync(0xffffffffu, bestJ, off);
+    const unsigned long long ok = __shfl_xor_sync(0xffffffffu, key, off);
+    if (ok != ~0ull && (key == ~0ull || oJ > bestJ || (oJ == bestJ && ok < key))) { bestJ = oJ; key = ok; }
+  }
+  if (lane != 0) return;
   unsigned long long idx = key & ((1ull << 40) - 1);
   const int n0 = b.node_off[r], N = h->n_orig;
   uint32_t reach[16], succ[16];
@@ -380,7 +390,7 @@ cudaError_t launch_linear(const LinArgs& a, int grid, cudaStream_t s) {
 #undef DYPLAN_LCASE
   }
   const long long nrec = (long long)a.in.R * a.L;
-  k_lemit<<<(unsigned)((nrec + 127) / 128), 128, 0, s>>>(a);
+  k_lemit<<<(unsigned)((nrec + 3) / 4), 128, 0, s>>>(a);   // one warp per record
   return cudaGetLastError();
 }
 

@@ -18,7 +18,7 @@ constexpr int kM0BlockInst = 128;   // payload instructions per loop iteration (
 constexpr int kM0Iters = 2048;
 constexpr int kM0WarpsPerSmsp = 8;
 
-enum M0Op { M0_FFMA = 0, M0_FADD_SAT, M0_FMUL, M0_FADD, M0_FMNMX3, M0_IADD3, M0_VIADDMNMX, M0_VIMNMX3, M0_IMAD, M0_LOP3, M0_MIX_SCREEN, M0_MIX_INT, M0_COUNT };
+enum M0Op { M0_FFMA = 0, M0_FADD_SAT, M0_FMUL, M0_FADD, M0_FMNMX3, M0_IADD3, M0_VIADDMNMX, M0_VIMNMX3, M0_IMAD, M0_LOP3, M0_MIX_SCREEN, M0_MIX_INT, M0_FFMA2, M0_FADD2, M0_FMUL2, M0_MIX_SCREEN2, M0_COUNT };
 
 template <int OP>
 __device__ __forceinline__ void m0_step(float (&f)[kM0Chains], int (&i)[kM0Chains], float c0, float c1, int k0, int k1) {
@@ -64,6 +64,40 @@ __device__ __forceinline__ void m0_mix_int(float (&f)[kM0Chains], int (&i)[kM0Ch
   }
 }
 
+// packed fp32 (sm_100: FFMA2 / FADD2 / FMUL2 work on an aligned register pair): kM0Chains / 2 chains of pairs
+__device__ __forceinline__ unsigned long long m0_pack(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void m0_unpack(unsigned long long v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+
+template <int OP>
+__device__ __forceinline__ void m0_step2(unsigned long long (&p)[kM0Chains / 2], unsigned long long c0, unsigned long long c1) {
+#pragma unroll
+  for (int c = 0; c < kM0Chains / 2; c++) {
+    if (OP == M0_FFMA2) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(p[c]) : "l"(c0), "l"(c1));
+    if (OP == M0_FADD2) asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(p[c]) : "l"(c1));
+    if (OP == M0_FMUL2) asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(p[c]) : "l"(c0));
+  }
+}
+
+// the screen with the product and the incumbent test of TWO evaluations in one FFMA2: per two (plan, level)
+// evaluations 2 FADD.SAT + 1 FFMA2 + 1 FMNMX3
+__device__ __forceinline__ void m0_mix_screen2(float (&f)[kM0Chains], float (&g)[kM0Chains], unsigned long long c00, unsigned long long cneg, float c1, float c2) {
+#pragma unroll
+  for (int c = 0; c < kM0Chains; c += 2) {
+    float x0, x1, z0, z1;
+    asm volatile("add.sat.f32 %0, %1, %2;" : "=f"(x0) : "f"(f[c]), "f"(c1));
+    asm volatile("add.sat.f32 %0, %1, %2;" : "=f"(x1) : "f"(f[c + 1]), "f"(c2));
+    unsigned long long z = m0_pack(x0, x1);
+    asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(z) : "l"(c00), "l"(cneg));
+    m0_unpack(z, z0, z1);
+    asm volatile("max.f32 %0, %0, %1, %2;" : "+f"(g[c >> 1]) : "f"(z0), "f"(z1));
+    f[c] = z0; f[c + 1] = z1;
+  }
+}
+
 template <int OP>
 __global__ void __launch_bounds__(kM0WarpsPerSmsp * 4 * 32, 1) k_m0(long long* __restrict__ stamps, float* __restrict__ sink, float c0, float c1, int k0, int k1) {
   float f[kM0Chains], g[kM0Chains];
@@ -80,6 +114,20 @@ __global__ void __launch_bounds__(kM0WarpsPerSmsp * 4 * 32, 1) k_m0(long long* _
       for (int rep = 0; rep < 6; rep++) m0_mix_screen(f, g, c0, c1, c0 + c1);
 #pragma unroll
       for (int c = 0; c < 8; c++) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[c]) : "f"(c0), "f"(c1));
+    } else if (OP == M0_MIX_SCREEN2) {
+      // 4 instructions per pair of chains -> 16 per call; 8 calls = 128
+      const unsigned long long c00 = m0_pack(c0, c0), cneg = m0_pack(-(c0 + c1), -c1);
+#pragma unroll
+      for (int rep = 0; rep < 8; rep++) m0_mix_screen2(f, g, c00, cneg, c1, c0 + c1);
+    } else if (OP == M0_FFMA2 || OP == M0_FADD2 || OP == M0_FMUL2) {
+      unsigned long long p[kM0Chains / 2];
+#pragma unroll
+      for (int c = 0; c < kM0Chains / 2; c++) p[c] = m0_pack(f[2 * c], f[2 * c + 1]);
+      const unsigned long long c00 = m0_pack(c0, c0), c11 = m0_pack(c1, c1);
+#pragma unroll
+      for (int rep = 0; rep < kM0BlockInst / (kM0Chains / 2); rep++) m0_step2<OP>(p, c00, c11);
+#pragma unroll
+      for (int c = 0; c < kM0Chains / 2; c++) m0_unpack(p[c], f[2 * c], f[2 * c + 1]);
     } else if (OP == M0_MIX_INT) {
       // 3 instructions per chain -> 24 per call; 5 calls + 8 payload = 128
 #pragma unroll
@@ -106,10 +154,12 @@ __global__ void __launch_bounds__(kM0WarpsPerSmsp * 4 * 32, 1) k_m0(long long* _
 typedef void (*m0_kernel_t)(long long*, float*, float, float, int, int);
 static const m0_kernel_t kM0Kernels[M0_COUNT] = {
     k_m0<M0_FFMA>, k_m0<M0_FADD_SAT>, k_m0<M0_FMUL>, k_m0<M0_FADD>, k_m0<M0_FMNMX3>, k_m0<M0_IADD3>,
-    k_m0<M0_VIADDMNMX>, k_m0<M0_VIMNMX3>, k_m0<M0_IMAD>, k_m0<M0_LOP3>, k_m0<M0_MIX_SCREEN>, k_m0<M0_MIX_INT>};
+    k_m0<M0_VIADDMNMX>, k_m0<M0_VIMNMX3>, k_m0<M0_IMAD>, k_m0<M0_LOP3>, k_m0<M0_MIX_SCREEN>, k_m0<M0_MIX_INT>,
+    k_m0<M0_FFMA2>, k_m0<M0_FADD2>, k_m0<M0_FMUL2>, k_m0<M0_MIX_SCREEN2>};
 static const char* const kM0Names[M0_COUNT] = {
     "FFMA", "FADD.SAT", "FMUL", "FADD", "FMNMX3", "IADD3", "VIADDMNMX", "VIMNMX3", "IMAD", "LOP3",
-    "mix: 2 FADD.SAT + 2 FFMA + 1 FMNMX3 (k_fscore screen)", "mix: IADD3 + FFMA + LOP3 (k_score screen)"};
+    "mix: 2 FADD.SAT + 2 FFMA + 1 FMNMX3 (k_fscore screen)", "mix: IADD3 + FFMA + LOP3 (k_score screen)",
+    "FFMA2 (packed: 2 FMA per lane)", "FADD2 (packed)", "FMUL2 (packed)", "mix: 2 FADD.SAT + 1 FFMA2 + 1 FMNMX3 (packed screen)"};
 
 int m0_count() { return M0_COUNT; }
 const char* m0_name(int op) { return (op >= 0 && op < M0_COUNT) ? kM0Names[op] : ""; }
