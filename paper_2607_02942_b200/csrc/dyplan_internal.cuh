@@ -185,7 +185,7 @@ constexpr int kLinBlobWords = kLinHdrWords + 2 * (16 * 16 + 4);   // header + (w
 struct LinHdr {
   int32_t status;                 // DYPLAN_ST_OK / _INVALID / _TOO_LARGE
   int32_t n_orig, n_int;          // real nodes, nodes incl. dummies (>= 2)
-  int32_t pad0;
+  float jmag;                     // bound on the magnitude of J and of every partial sum of it, over the request's plans and the call's levels
   unsigned long long outer_total; // prod_{i>=3} K_i
   unsigned long long pad1;
   int32_t K[16];                  // options per internal node (1 for dummies)

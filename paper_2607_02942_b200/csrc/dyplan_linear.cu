@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
     }
     if (st == DYPLAN_ST_OK && dsum > (1ull << 22)) st = DYPLAN_ST_TOO_LARGE;
   }
-  h->status = st; h->n_orig = N; h->n_int = N < 3 ? 3 : N; h->pad0 = 0;
+  h->status = st; h->n_orig = N; h->n_int = N < 3 ? 3 : N; h->jmag = 0.0f;
   if (st != DYPLAN_ST_OK) {
     h->outer_total = 0;
     for (int l = 0; l < L; l++) {
@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
   unsigned long long stride = 1, outer = 1;
   int slot = 0;
   const int Np = N < 3 ? 3 : N;
+  float mag_w = 0.0f, mag_d = 0.0f;   // sum over the nodes of max_k |w| and of max_k d
   for (int n = 0; n < 16; n++) {
     if (n < N) {
       const int ob = b.opt_off[n0 + n], K = b.opt_off[n0 + n + 1] - ob;
@@ -98,6 +99,9 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
         t_wd[slot + k] = make_float2((float)(rho * q - (double)a.p.lambda_f * v * (1.0 - q) - (double)a.p.lambda_c * (double)a.cost[ob + k]),
                                      (float)b.lat_us[ob + k]);
       }
+      float mw = 0.0f, md = 0.0f;
+      for (int k = 0; k < K; k++) { mw = fmaxf(mw, fabsf(t_wd[slot + k].x)); md = fmaxf(md, t_wd[slot + k].y); }
+      mag_w += mw; mag_d += md;
       slot += K;
       stride *= (unsigned long long)K;
       if (n >= 3) outer *= (unsigned long long)K;
@@ -107,6 +111,11 @@ __global__ void __launch_bounds__(128) k_lstage(LinArgs a) {
     }
   }
   h->outer_total = outer;
+  {
+    float lv = 0.0f;
+    for (int l = 0; l < L; l++) lv = fmaxf(lv, a.levels[l]);
+    h->jmag = mag_w + (a.p.lambda_l + a.p.lambda_ld * lv) * mag_d;
+  }
   atomicAdd(a.plans, P);
 }
 
@@ -139,6 +148,21 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
   float w0[K0P], d0[K0P];         // node 0's tables in registers (padding options: w = -1e30, never an incumbent)
 #pragma unroll
   for (int k = 0; k < K0P; k++) { const float2 wd = t_wd[k < K0 ? k : 0]; w0[k] = k < K0 ? wd.x : -1e30f; d0[k] = k < K0 ? wd.y : 0.0f; }
+  // Tabled screen (when the table fits the register file): J - best = [cl D1 + W1 - best] + [cl d0 + w0] + lambda_l m,
+  // the second bracket a constant per (option of node 0, level), the first one per (group, level).  Per evaluation that
+  // leaves one FFMA and half an FMNMX3; the first bracket is added to the per-level maxima once per group.  The sum is
+  // associated differently from J32 (the pure function of the plan the re-walk computes), so the screen passes
+  // everything within eps of the incumbent: both chains are at most 5 roundings of partial sums no larger than jmag
+  // (2^-24 each, under 2^-20 jmag together); eps = 2^-19 jmag.  The re-walk alone decides what replaces an incumbent.
+  constexpr bool kTab = K0P * LT <= 32;
+  float E[kTab ? K0P : 1][LT];
+  if (kTab) {
+#pragma unroll
+    for (int k = 0; k < K0P; k++)
+#pragma unroll
+      for (int l = 0; l < LT; l++) E[k][l] = fmaf(cl[l], d0[k], w0[k]);
+  }
+  const float neg_eps = -(h->jmag * (1.0f / 524288.0f));
   float best[LT];                 // the lane's incumbent J per level and, among the plans attaining it, min (T << 40 | idx)
   unsigned long long kmin[LT];
 #pragma unroll
@@ -212,6 +236,21 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
         const unsigned long long idx1 = idx2 + (unsigned long long)k1 * st1;
         // screen: h > = 0 iff some (plan, level) of the group ties or beats the lane's incumbent (J - best has an exact sign)
         float h = -1.0f;
+        if (kTab) {
+          float hm[LT];
+#pragma unroll
+          for (int l = 0; l < LT; l++) hm[l] = -INFINITY;
+#pragma unroll
+          for (int k0 = 0; k0 + 1 < K0P; k0 += 2) {
+            const float ma = fminf(R1, ap - d0[k0]), mb = fminf(R1, ap - d0[k0 + 1]);   // least slack = -T
+#pragma unroll
+            for (int l = 0; l < LT; l++) hm[l] = fmaxf(hm[l], fmaxf(fmaf(lam_l, ma, E[k0][l]), fmaf(lam_l, mb, E[k0 + 1][l])));
+          }
+          float hh = -INFINITY;
+#pragma unroll
+          for (int l = 0; l < LT; l++) hh = fmaxf(hh, hm[l] + (fmaf(cl[l], D1, W1) - best[l]));
+          h = hh >= neg_eps ? 0.0f : -1.0f;
+        } else
 #pragma unroll
         for (int k0 = 0; k0 < K0P; k0++) {
           const float m = fminf(R1, ap - d0[k0]);        // least slack = -T
@@ -265,7 +304,7 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
 }
 
 template <int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
-__global__ void __launch_bounds__(128) k_lscore(LinArgs a) {
+__global__ void __launch_bounds__(128, (LT <= 4 ? 4 : 3)) k_lscore(LinArgs a) {
   __shared__ __align__(16) uint32_t s_blob[4][kLinBlobWords];
   __shared__ float s_cl[8];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;

@@ -212,3 +212,30 @@ def test_linear_full_size_cfg1_shapes(dy):
     ref = lo.compile(sub.batch, csub, p, levels)
     gs = {k: v.reshape(256, -1)[rows].reshape(-1) for k, v in g.items()}
     check(lo, sub.batch, csub, p, levels, gs, ref)
+
+
+@pytest.mark.parametrize("seed,levels", [(211, [0.0, 1.5, 3.0]), (212, [0.0, 0.5, 1.0, 2.0]), (213, [0.0, 0.5, 1.0, 2.0, 4.0, 8.0])])
+def test_linear_exact_ties_take_the_lowest_key(dy, seed, levels):
+    # Option 1 of every node is a copy of option 0: every plan has 2^(#nodes) exact twins (same J in fp32 and in fp64,
+    # same T), so the winner is decided by the canonical index alone.  The scorer's screen only has to pass everything
+    # that ties or beats the incumbent (its own sum is associated differently from J32 and is given a margin); the exact
+    # re-walk decides.  A screen that dropped ties, or a reduction that lost the key order, would pick an option 1.
+    from oracle import linear as lo
+    batch, cost = case(seed, R=24, nmin=2, nmax=7, kmin=2, kmax=6)
+    for n in range(batch.NN):
+        o = int(batch.opt_off[n])
+        for a in (batch.lat_us, batch.acc, batch.demand, batch.backend, batch.model, cost):
+            a[o + 1] = a[o]
+    p = f32(P0)
+    lv = [float(np.float32(x)) for x in levels]
+    g, _ = run_gpu(dy, batch, cost, p, levels)
+    ref = lo.compile(batch, cost, p, lv)
+    check(lo, batch, cost, p, lv, g, ref)
+    ch = g["choice"].reshape(-1, 16)
+    ok = g["status"] == 0
+    assert ok.all()
+    assert (ch[ok] != 1).all(), "a twin with a higher canonical index won a tie"
+    # where the chosen plan's fp64 J equals the oracle's optimum bit for bit, the plan is the oracle's
+    exact = g["corr64"] == ref["J"]
+    assert exact.sum() >= 0.8 * ok.sum()
+    assert np.array_equal(g["plan_idx"][exact], np.asarray(ref["plan_idx"], np.uint64)[exact])
