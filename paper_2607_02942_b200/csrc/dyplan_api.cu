@@ -257,7 +257,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
   a.max_items = max_items;
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
-  a.small_split = a.small_mode ? (4 * ctx->sm_count / (int)in->R > 1 ? 4 * ctx->sm_count / (int)in->R : 1) : 1;
+  a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
 
   CK(launch_stage(a, stream));
   int launches = 1;
@@ -863,7 +863,7 @@ extern "C" int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, in
   memset(&a, 0, sizeof(a));
   a.in = *in; a.out = *out; a.L = L; a.mult = mult_pm; a.ctx_flags = ctx->flags;
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
-  a.small_split = a.small_mode ? (4 * ctx->sm_count / (int)in->R > 1 ? 4 * ctx->sm_count / (int)in->R : 1) : 1;
+  a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
   StaticCarver sc{base};
   a.blob = sc.take<uint32_t>(R * blob_stride_words(L));
   a.item_off = sc.take<uint32_t>(2 * (R + 1)); a.item_off_f = a.item_off + (R + 1);

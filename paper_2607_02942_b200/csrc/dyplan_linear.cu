@@ -304,7 +304,7 @@ __device__ __noinline__ void litem(const uint32_t* __restrict__ sb, const LinArg
 }
 
 template <int LT>   // LT: level count padded to 1,2,3,4,6,8 (padded levels repeat a zero weight and are dropped)
-__global__ void __launch_bounds__(128, (LT <= 4 ? 4 : 3)) k_lscore(LinArgs a) {
+__global__ void __launch_bounds__(128, (LT <= 4 ? 4 : 3)) k_lscore(const __grid_constant__ LinArgs a) {
   __shared__ __align__(16) uint32_t s_blob[4][kLinBlobWords];
   __shared__ float s_cl[8];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;

@@ -13,10 +13,163 @@
 
 namespace dyplan {
 
-// (not inlined: only the last block of a request runs it)
-__device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) { emit_record(a, h, r, l, w); }
+// S6 for one record by one WARP (only the last block of a request runs it).  Same outputs as emit_record
+// (dyplan_common.cuh), which one thread walks node by node with two dependent global loads and a 64-bit division per
+// node; here lane n takes node n -- option counts, the digit of the winner's canonical index, the option's annotations
+// -- so the record costs two round trips to L2 instead of two per node.  C64 is still the product in node order, by
+// one lane, without contraction (definition 4; matches the plain definition bit for bit).
+__device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) {
+  const int lane = threadIdx.x & 31;
+  if (w.idx == kNoIdx) {   // warp-uniform
+    if (lane == 0) emit_record(a, h, r, l, w);
+    return;
+  }
+  const dyplan_batch& b = a.in;
+  const dyplan_bundle& o = a.out;
+  const int B = b.B, M = b.M;
+  const long long rec = r * a.L + l;
+  const int n0 = h->n0, N = h->n_orig;
+  int ob = 0;
+  unsigned long long K = 1;
+  if (lane < N) { ob = b.opt_off[n0 + lane]; K = (unsigned long long)(b.opt_off[n0 + lane + 1] - ob); }
+  unsigned long long stride = K;   // inclusive prefix product over the lanes, then shifted: stride of node `lane`
+#pragma unroll
+  for (int off = 1; off < 16; off <<= 1) {
+    const unsigned long long t = __shfl_up_sync(0xffffffffu, stride, off);
+    if (lane >= off) stride *= t;
+  }
+  stride = __shfl_up_sync(0xffffffffu, stride, 1);
+  if (lane == 0) stride = 1;
+  const int k = lane < N ? (int)((w.idx / stride) % K) : 0;
+  double f = 1.0;
+  int be = 0, mo = 0, dm = 0;
+  if (lane < 16) o.choice[rec * 16 + lane] = lane < N ? (uint8_t)k : (uint8_t)0xFF;
+  if (lane < N && !((h->skip_mask >> lane) & 1)) {
+    const int op = ob + k;
+    f = __dsub_rn(1.0, __dmul_rn((double)b.vuln[n0 + lane], __dsub_rn(1.0, (double)b.acc[op])));
+    be = b.backend[op]; mo = b.model[op]; dm = b.demand[op];
+  }
+  double c = 1.0;
+  int D[DYPLAN_MAX_BACKENDS], Dm[DYPLAN_MAX_MODELS];
+#pragma unroll
+  for (int i = 0; i < DYPLAN_MAX_BACKENDS; i++) D[i] = 0;
+#pragma unroll
+  for (int i = 0; i < DYPLAN_MAX_MODELS; i++) Dm[i] = 0;
+  for (int n = 0; n < N; n++) {   // node order (skipped nodes carry f = 1, demand 0)
+    c = __dmul_rn(c, __shfl_sync(0xffffffffu, f, n));
+    const int bn = __shfl_sync(0xffffffffu, be, n), mn = __shfl_sync(0xffffffffu, mo, n), dn = __shfl_sync(0xffffffffu, dm, n);
+#pragma unroll
+    for (int i = 0; i < DYPLAN_MAX_BACKENDS; i++) D[i] += (i == bn) ? dn : 0;
+#pragma unroll
+    for (int i = 0; i < DYPLAN_MAX_MODELS; i++) Dm[i] += (i == mn) ? dn : 0;
+  }
+  if (lane != 0) return;
+  int dmod = 0, dbest = Dm[0];
+#pragma unroll
+  for (int m = 1; m < DYPLAN_MAX_MODELS; m++) if (m < M && Dm[m] > dbest) { dbest = Dm[m]; dmod = m; }   // ties -> lowest id (reading Q13)
+  o.plan_idx[rec] = w.idx;
+  o.corr[rec] = w.C;
+  if (o.corr64) o.corr64[rec] = c;
+  o.lat[rec] = w.T;
+#pragma unroll
+  for (int bb = 0; bb < DYPLAN_MAX_BACKENDS; bb++) if (bb < B) o.dem[rec * B + bb] = D[bb];
+  o.dom_model[rec] = (uint8_t)dmod;
+  o.status[rec] = DYPLAN_ST_OK;
+}
 
-__global__ void __launch_bounds__(kSmallThreads) k_small(const CallArgs a) {
+// Plans [p, pe) of one request, from scratch, one after the other: NPB bounds the node count, so that the digits, the
+// slots and the slacks are registers (a node loop with a run-time bound put them in local memory: 0.7 M local accesses
+// per launch on configs[0]).  deps(i) only holds nodes j > i and is the same for every thread of the block, so the slack
+// recurrence is a chain of predicated minima with uniform predicates.  The canonical index is only formed for a plan
+// that is not already worse than the incumbent on (C, T).
+template <int NPB>
+__device__ __forceinline__ void small_walk(const uint32_t* __restrict__ sb, const int L, const bool caps, uint32_t p, const uint32_t pe, Best (&best)[DYPLAN_MAX_LEVELS]) {
+  const ReqHdr* h = (const ReqHdr*)sb;
+  const int nsp = h->nslots_pad, Np = h->n_int, slo = h->slo;
+  const int* s_lat = (const int*)(sb + kHdrWords + kDem0bWords);   // [slot][L]
+  const float* s_f = (const float*)(s_lat + nsp * L);
+  const int* s_dem = (const int*)(s_f + nsp);
+  const int* s_be = s_dem + nsp;
+  int dig[NPB], rad[NPB], ob[NPB];
+  uint32_t dep[NPB];
+  {
+    uint32_t q = p;
+#pragma unroll
+    for (int i = 0; i < NPB; i++) {
+      rad[i] = i < Np ? (i == 0 ? h->K0 : (i == 1 ? h->K1 : h->Kp[i])) : 1;
+      ob[i] = i < Np ? h->optbase[i] : 0;
+      dep[i] = i < Np ? h->deps[i] : 0u;
+      dig[i] = (int)(q % (uint32_t)rad[i]);
+      q /= (uint32_t)rad[i];
+    }
+  }
+  for (; p < pe; p++) {
+    // definition 4 (as every scorer rounds it: the fp32 product from the last internal node down), 5 and 1
+    float C = 1.0f;
+    int D[DYPLAN_MAX_BACKENDS];
+#pragma unroll
+    for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) D[b] = 0;
+    int sl[NPB];   // slot of node i's option
+#pragma unroll
+    for (int i = NPB - 1; i >= 0; --i) {
+      sl[i] = ob[i] + dig[i];
+      if (i < Np) {
+        C = __fmul_rn(C, s_f[sl[i]]);
+        if (caps) {
+          const int be = s_be[sl[i]] & 7, dm = s_dem[sl[i]];
+#pragma unroll
+          for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) D[b] += (b == be) ? dm : 0;
+        }
+      }
+    }
+    bool capok = true;
+    if (caps) {
+#pragma unroll
+      for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) capok = capok && D[b] <= h->cap[b];
+    }
+    if (capok) {
+      unsigned long long idx = kNoIdx;   // formed on first use
+#pragma unroll
+      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+        if (l < L) {
+          // definitions 2-3 in slack form: u[i] = min(SLO, min_{j in deps(i)} u[j]) - d_l(i, k_i), T = SLO - min_i u[i]
+          int u[NPB];
+          int ms = slo;
+#pragma unroll
+          for (int i = NPB - 1; i >= 0; --i) {
+            u[i] = slo;
+            if (i < Np) {
+              int m = slo;
+#pragma unroll
+              for (int j = i + 1; j < NPB; j++) if ((dep[i] >> j) & 1u) m = min(m, u[j]);
+              const int v = m - s_lat[sl[i] * L + l];
+              u[i] = v;
+              ms = min(ms, v);
+            }
+          }
+          const int T = slo - ms;
+          if (ms >= 0 && (best[l].idx == kNoIdx || C > best[l].C || (C == best[l].C && T <= best[l].T))) {
+            if (idx == kNoIdx) {
+              idx = h->base_idx;
+#pragma unroll
+              for (int i = 0; i < NPB; i++) if (i < Np) idx += (unsigned long long)dig[i] * h->stride[i];
+            }
+            if (better(C, T, idx, best[l])) { best[l].C = C; best[l].T = T; best[l].idx = idx; }
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NPB; i++) {   // odometer
+      if (++dig[i] < rad[i]) break;
+      dig[i] = 0;
+    }
+  }
+}
+
+// (`a` is a __grid_constant__: the not-inlined emit_small takes it by reference, and without the qualifier every thread
+// first copied the 1.2 KB argument block to its local memory -- 100 STL.128 per warp, 126 MB of local stores per launch)
+__global__ void __launch_bounds__(kSmallThreads, 4) k_small(const __grid_constant__ CallArgs a) {
   __shared__ __align__(16) uint32_t sb[kMaxBlobWords];
   __shared__ Best s_red[DYPLAN_MAX_LEVELS][kSmallThreads / 32];
   __shared__ uint32_t s_last;
@@ -26,79 +179,38 @@ __global__ void __launch_bounds__(kSmallThreads) k_small(const CallArgs a) {
   const int part = blockIdx.x % split;
   const int L = a.L;
   const uint32_t* gblob = a.blob + (size_t)r * blob_stride_words(L);
-  const ReqHdr* gh = (const ReqHdr*)gblob;
-  if (gh->status != DYPLAN_ST_OK || gh->klass != kClassSmall) return;   // block-uniform
-  const int words = kHdrWords + kDem0bWords + gh->nslots_pad * (L + 3);
-  for (int i = tid; i < words; i += kSmallThreads) sb[i] = gblob[i];
+  // the header says how long the blob is, but reading it first would put two round trips to L2 in front of every
+  // block: the first 5 x 128 words (header, dem0b and 35 slots at 3 levels) are fetched unconditionally, the rest after
+  constexpr int kFirst = 5 * kSmallThreads;
+#pragma unroll
+  for (int i = 0; i < 5; i++) sb[tid + i * kSmallThreads] = gblob[tid + i * kSmallThreads];
   __syncthreads();
   const ReqHdr* h = (const ReqHdr*)sb;
-  const int nsp = h->nslots_pad, Np = h->n_int, slo = h->slo;
-  const int* s_lat = (const int*)(sb + kHdrWords + kDem0bWords);   // [slot][L]
-  const float* s_f = (const float*)(s_lat + nsp * L);
-  const int* s_dem = (const int*)(s_f + nsp);
-  const int* s_be = s_dem + nsp;
+  if (h->status != DYPLAN_ST_OK || h->klass != kClassSmall) return;   // block-uniform
+  const int words = kHdrWords + kDem0bWords + h->nslots_pad * (L + 3);
+  if (words > kFirst) {   // block-uniform
+    for (int i = kFirst + tid; i < words; i += kSmallThreads) sb[i] = gblob[i];
+    __syncthreads();
+  }
+  const int Np = h->n_int;
 
   // this thread's contiguous range of enumerated plans (internal mixed radix, node 0 fastest); P <= 2^21
   const uint32_t P = (uint32_t)(h->outer_total * (unsigned long long)(h->K0 * h->K1));
   const uint32_t nthr = (uint32_t)split * kSmallThreads;
   const uint32_t chunk = (P + nthr - 1) / nthr;
   const uint32_t gt = (uint32_t)part * kSmallThreads + tid;
-  uint32_t p = gt * chunk < P ? gt * chunk : P;
+  const uint32_t p = gt * chunk < P ? gt * chunk : P;
   const uint32_t pe = p + chunk < P ? p + chunk : P;
-  int dig[16], rad[16];
-  {
-    uint32_t q = p;
-    for (int i = 0; i < Np; i++) {
-      rad[i] = i == 0 ? h->K0 : (i == 1 ? h->K1 : h->Kp[i]);
-      dig[i] = (int)(q % (uint32_t)rad[i]);
-      q /= (uint32_t)rad[i];
-    }
-  }
   Best best[DYPLAN_MAX_LEVELS];
 #pragma unroll
   for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) { best[l].C = -1.0f; best[l].T = INT32_MAX; best[l].idx = kNoIdx; }
-
-  for (; p < pe; p++) {
-    // definition 4 (as every scorer rounds it), 5 and 1
-    float C = 1.0f;
-    int D[DYPLAN_MAX_BACKENDS];
-#pragma unroll
-    for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) D[b] = 0;
-    unsigned long long idx = h->base_idx;
-    for (int i = Np - 1; i >= 0; --i) {
-      const int slot = h->optbase[i] + dig[i];
-      C = __fmul_rn(C, s_f[slot]);
-      const int be = s_be[slot] & 7, dm = s_dem[slot];
-#pragma unroll
-      for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) D[b] += (b == be) ? dm : 0;
-      idx += (unsigned long long)dig[i] * h->stride[i];
-    }
-    bool capok = true;
-#pragma unroll
-    for (int b = 0; b < DYPLAN_MAX_BACKENDS; b++) capok = capok && D[b] <= h->cap[b];
-    if (capok) {
-#pragma unroll
-      for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
-        if (l < L) {
-          // definitions 2-3 in slack form: u[i] = min(SLO, min_{j in deps(i)} u[j]) - d_l(i, k_i), T = SLO - min_i u[i]
-          int u[16];
-          int ms = slo;
-          for (int i = Np - 1; i >= 0; --i) {
-            int m = slo;
-            for (uint32_t dm = h->deps[i]; dm; dm &= dm - 1) m = min(m, u[__ffs(dm) - 1]);
-            const int v = m - s_lat[(h->optbase[i] + dig[i]) * L + l];
-            u[i] = v;
-            ms = min(ms, v);
-          }
-          if (ms >= 0 && better(C, slo - ms, idx, best[l])) { best[l].C = C; best[l].T = slo - ms; best[l].idx = idx; }
-        }
-      }
-    }
-    for (int i = 0; i < Np; i++) {   // odometer
-      if (++dig[i] < rad[i]) break;
-      dig[i] = 0;
-    }
-  }
+  // (one instantiation per bound on the node count: digits, slots and slacks stay in registers)
+  const bool caps = a.in.cap != nullptr;
+  if (Np <= 4) small_walk<4>(sb, L, caps, p, pe, best);
+  else if (Np <= 6) small_walk<6>(sb, L, caps, p, pe, best);
+  else if (Np <= 8) small_walk<8>(sb, L, caps, p, pe, best);
+  else if (Np <= 12) small_walk<12>(sb, L, caps, p, pe, best);
+  else small_walk<16>(sb, L, caps, p, pe, best);
 
   // ---- block arg-best per level, one record per (request, part, level) ----
 #pragma unroll
@@ -123,17 +235,35 @@ __global__ void __launch_bounds__(kSmallThreads) k_small(const CallArgs a) {
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  for (int l = wid; l < L; l += kSmallThreads / 32) {
-    // ---- last block of this request: a warp reduces one level's records and emits (S6) ----
+  // ---- last block of this request: the records of all parts, every level (S6).  All 128 threads fetch (the loads of
+  // one thread are independent: four in flight), then warp shuffles, shared memory, and warp l emits level l ----
+#pragma unroll
+  for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
+    if (l >= L) break;
     Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
-    for (int j = lane; j < split; j += 32) {
-      const float4 raw = __ldcg((const float4*)&part_rec[(size_t)j * L + l]);
-      Best o; o.C = raw.x; o.T = __float_as_int(raw.y);
-      o.idx = ((unsigned long long)__float_as_uint(raw.w) << 32) | (unsigned long long)__float_as_uint(raw.z);
-      if (better(o.C, o.T, o.idx, v)) v = o;
+    for (int j0 = tid; j0 < split; j0 += 4 * kSmallThreads) {
+      float4 raw[4];
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        const int j = j0 + q * kSmallThreads;
+        raw[q] = j < split ? __ldcg((const float4*)&part_rec[(size_t)j * L + l]) : make_float4(-1.0f, __int_as_float(INT32_MAX), __uint_as_float(0xffffffffu), __uint_as_float(0xffffffffu));
+      }
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        Best o; o.C = raw[q].x; o.T = __float_as_int(raw[q].y);
+        o.idx = ((unsigned long long)__float_as_uint(raw[q].w) << 32) | (unsigned long long)__float_as_uint(raw[q].z);
+        if (better(o.C, o.T, o.idx, v)) v = o;
+      }
     }
     v = warp_best(v);
-    if (lane == 0) emit_small(a, h, r, l, v);
+    if (lane == 0) s_red[l][wid] = v;
+  }
+  __syncthreads();
+  for (int l = wid; l < L; l += kSmallThreads / 32) {
+    Best v = s_red[l][0];
+#pragma unroll
+    for (int w = 1; w < kSmallThreads / 32; w++) { const Best o = s_red[l][w]; if (better(o.C, o.T, o.idx, v)) v = o; }
+    emit_small(a, h, r, l, v);
   }
   if (tid == 0) { atomicAdd(&a.st->total_plans, (unsigned long long)P); atomicAdd(&a.st->small_requests, 1u); }   // (k_plan sets the totals again when the general scorers run too)
 }

@@ -525,6 +525,38 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   const int tid = threadIdx.x;
   const long long R = a.in.R;
   const size_t blob_stride = blob_stride_words(a.L);
+  if (a.small_mode) {
+    // a small call (R <= kSmallMaxR <= 32) whose requests k_small has all taken: nothing to plan.  One warp settles it
+    // (the scans and reductions below cost 10 us of fixed latency, a tenth of an admission-time compile)
+    __shared__ int s_other;
+    if (tid == 0) s_other = 0;
+    __syncthreads();
+    unsigned long long pl = 0;
+    uint32_t is_small = 0;
+    if (tid < R) {
+      const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)tid * blob_stride);
+      if (h->status == DYPLAN_ST_OK) {
+        if (h->klass == kClassSmall) { is_small = 1; pl = h->outer_total * (unsigned long long)(h->K0 * h->K1); }
+        else s_other = 1;
+      }
+    }
+    __syncthreads();
+    if (!s_other) {   // block-uniform
+      if (tid < 32) {
+#pragma unroll
+        for (int off = 16; off; off >>= 1) { pl += __shfl_xor_sync(0xffffffffu, pl, off); is_small += __shfl_xor_sync(0xffffffffu, is_small, off); }
+      }
+      if (tid <= R) { a.item_off[tid] = 0; a.item_off_f[tid] = 0; }
+      if (tid == 0) {
+        CallState* st = a.st;
+        st->total_outer = 0; st->total_plans = pl; st->per_item_outer = kBlock; st->per_item_outer_f = 32;
+        st->slow_steps = 0; st->bound_skipped = 0;
+        st->total_items = 0; st->next_item = 0; st->total_items_f = 0; st->next_item_f = 0;
+        st->fast_requests = 0; st->small_call_f = 1u; st->tail_start_f = 0xffffffffu; st->approx_requests = 0; st->small_requests = is_small; st->pad0 = 0;
+      }
+      return;
+    }
+  }
   const long long chunk = (R + 1023) / 1024;
   const long long r0 = tid * chunk, r1 = r0 + chunk < R ? r0 + chunk : R;
   unsigned long long so = 0, sf = 0, sp = 0, mxf = 0;
