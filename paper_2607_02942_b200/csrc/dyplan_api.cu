@@ -205,7 +205,7 @@ static int check_bundle(const dyplan_bundle* o) {
 // call is one k_small takes, so the batched scorers are not launched at all
 static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult, const uint32_t* dispatched,
                      const uint8_t* fixed_choice, uint32_t flags, bool is_replan, dyplan_bundle* out, cudaStream_t stream,
-                     bool all_small = false) {
+                     bool all_small = false, const void* img_src = nullptr, void* img_dst = nullptr, size_t img_bytes = 0) {
   if (!ctx) return DYPLAN_ERR_NULL;
   int rc = check_batch(in, true);
   if (rc) return rc;
@@ -256,6 +256,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f;
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
   a.max_items = max_items;
+  a.img_src = (const uint4*)img_src; a.img_dst = (uint4*)img_dst; a.img_vec = (uint32_t)((img_bytes + 15) / 16);
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
   a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
 
@@ -548,6 +549,7 @@ size_t arena_bytes(const HostPlan& p) {
 // inputs are packed into a pinned image of the arena and travel as ONE copy each way; larger calls copy each array
 // straight from the caller's buffer (packing 27 MB on the host would cost more than it saves).
 constexpr size_t kStageBytes = 256 << 10;
+constexpr size_t kZeroCopyBytes = 8 << 10;   // input images up to this size are fetched by k_stage itself (no DMA copies)
 #define H2D(dst, src, n, T)                                                                            \
   do {                                                                                                 \
     dst = ar.take<T>(n);                                                                               \
@@ -648,10 +650,22 @@ static int solve_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const 
   int32_t* dmult; uint32_t* ddisp = nullptr; uint8_t* dfix = nullptr;
   H2D(dmult, mult, is_replan ? (size_t)in->R * in->B : (size_t)L * in->B, int32_t);
   if (is_replan) { H2D(ddisp, dispatched, (size_t)in->R, uint32_t); H2D(dfix, fixed_choice, (size_t)in->NN, uint8_t); }
-  if (ar.stage) CK(cudaMemcpyAsync(ar.base, ar.stage, ar.off, cudaMemcpyHostToDevice, s));   // the whole input image, once
+  // A tiny call (one admission-time compile is a few hundred bytes in, a few hundred out) does not use the copy engine at
+  // all: k_stage fetches the image from the pinned buffer itself and the kernels store the records straight into it
+  // (pinned memory is device-visible at the same address); what is left of the call is two launches and a synchronise.
+  const size_t in_bytes = ar.off;
+  const bool zero_copy = ar.stage && in_bytes <= kZeroCopyBytes;
+  if (ar.stage && !zero_copy) CK(cudaMemcpyAsync(ar.base, ar.stage, ar.off, cudaMemcpyHostToDevice, s));   // the whole input image, once
   const size_t out_begin = (ar.off + 255) & ~(size_t)255;
   dyplan_bundle dout;
   bundle_alloc(ar, hp.nrec, hp.B, out->corr64 != nullptr, &dout);
+  if (zero_copy) {   // the records' home is the pinned image
+    const ptrdiff_t sh = ar.stage - ar.base;
+    dout.plan_idx = (uint64_t*)((char*)dout.plan_idx + sh); dout.choice = (uint8_t*)((char*)dout.choice + sh);
+    dout.corr = (float*)((char*)dout.corr + sh); if (dout.corr64) dout.corr64 = (double*)((char*)dout.corr64 + sh);
+    dout.lat = (int32_t*)((char*)dout.lat + sh); dout.dem = (int32_t*)((char*)dout.dem + sh);
+    dout.dom_model = (uint8_t*)((char*)dout.dom_model + sh); dout.status = (uint8_t*)((char*)dout.status + sh);
+  }
   // every request small enough for k_small (an upper bound of what k_stage will find: pinned nodes only shrink it)?
   bool all_small = in->R <= kSmallMaxR;
   for (int32_t r = 0; r < in->R && all_small; r++) {
@@ -664,8 +678,12 @@ static int solve_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const 
       if (p * (unsigned long long)L > kSmallMaxEvals) all_small = false;
     }
   }
-  if ((rc = run_solve(ctx, &d, L, dmult, ddisp, dfix, flags, is_replan, &dout, s, all_small))) return rc;
-  if (ar.stage) {
+  if ((rc = run_solve(ctx, &d, L, dmult, ddisp, dfix, flags, is_replan, &dout, s, all_small, zero_copy ? ar.stage : nullptr,
+                      zero_copy ? ar.base : nullptr, zero_copy ? in_bytes : 0))) return rc;
+  if (zero_copy) {
+    CK(cudaStreamSynchronize(s));
+    if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h, ar.stage, ar.stage))) return rc;
+  } else if (ar.stage) {
     CK(cudaMemcpyAsync(ar.stage + out_begin, ar.base + out_begin, ar.off - out_begin, cudaMemcpyDeviceToHost, s));   // every record, once
     CK(cudaStreamSynchronize(s));
     if ((rc = bundle_to_host(ctx, &dout, out, hp.nrec, hp.B, s, d2h, ar.stage, ar.base))) return rc;

@@ -124,6 +124,9 @@ struct CallArgs {                   // passed by value to the kernels
   uint32_t flags;
   uint32_t ctx_flags;               // DYPLAN_PRUNE_DOMINATED | DYPLAN_PRUNE_BOUNDS (dyplan_set_flags)
   int32_t is_replan;
+  const uint4* img_src;             // tiny *_host calls: the packed input image in pinned host memory (device-visible), or null
+  uint4* img_dst;                   //   ... and where k_stage copies it in the device arena (the batch pointers point there)
+  uint32_t img_vec;                 //   ... its length in 16-byte words
   int32_t small_mode;               // R <= kSmallMaxR: requests of at most kSmallMaxEvals evaluations are staged for k_small
   int32_t small_split;              // blocks per request in k_small (about 4 blocks per SM over the call)
   // scratch

@@ -64,6 +64,13 @@ __device__ uint32_t dominance_keep(const dyplan_batch& b, int o0, int K, float v
 // One warp per request.
 __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
   const int lane = threadIdx.x & 31;
+  if (a.img_src) {
+    // a tiny *_host call: its inputs (a few hundred bytes) arrive as one image in pinned host memory, and every block
+    // fetches the whole of it itself (one round trip over the host link; blocks write identical bytes) instead of the
+    // call paying a DMA copy and its stream-order hand-over in front of this kernel
+    for (uint32_t i = threadIdx.x; i < a.img_vec; i += blockDim.x) a.img_dst[i] = a.img_src[i];
+    __syncthreads();
+  }
   const long long r = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const dyplan_batch& b = a.in;
   if (r >= b.R) return;
