@@ -1,5 +1,6 @@
 // dyplan_api.cu -- the C ABI of include/dyplan.h: argument checks, scratch management, kernel sequencing.
 // No arithmetic of the method lives here; every step of the path runs in the kernels.
+#include <math.h>
 #include <stdio.h>
 #include <string.h>
 
@@ -260,6 +261,13 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
   a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
 
+  // The plain (device-pointer) call cannot see the option counts, but the sizes in the struct bound them: a request's
+  // plan count is at most the product of ALL option counts of the batch, which is at most (KK / NN)^NN (AM-GM; exact
+  // for one request with equal counts).  When that bound times L fits k_small's limit, every request that k_stage
+  // accepts is small, and the batched scorers have nothing to do: their four launches (about 20 us) are not issued.
+  if (a.small_mode && !all_small && in->NN > 0 && in->KK >= in->NN &&
+      (double)in->NN * log2((double)in->KK / (double)in->NN) + log2((double)L) <= 20.99)
+    all_small = true;
   CK(launch_stage(a, stream));
   int launches = 1;
   const bool only_small = a.small_mode && all_small;
