@@ -586,6 +586,7 @@ def run_linear(args, rank: int, world: int, local_rank: int):
         return
     aops = 2.0 + 5.0 / L      # per (plan, level): FFMA + compare; per plan: add-min (2), two sums, one FFMA
     k_eval_s = evals * args.steps / (tot_ms * 1e-3)
+    lin_traffic, lin_traffic_src = committed_traffic(f"linear_cfg{cfg}") if args.requests is None else (None, None)
     line = {
         "metric": METRIC, "value": whole_job_rate(evals, world, args.steps, tot_ms) / 1e9, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps, "higher_is_better": True,
@@ -599,7 +600,7 @@ def run_linear(args, rank: int, world: int, local_rank: int):
         "gpu_launches": st["launches"] * args.steps, "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": "k_lscore", "achieved": k_eval_s * aops / 1e12, "peak": peaks["peak"],
                      "unit": "Tinst/s", "frac": k_eval_s * aops / 1e12 / peaks["peak"], "peak_nominal": peaks["peak_nominal"],
-                     "traffic": None, "ops_per_eval": aops, "kernel_ms": st["score_ms"]},
+                     "traffic": lin_traffic, "traffic_source": lin_traffic_src, "ops_per_eval": aops, "kernel_ms": st["score_ms"]},
     }
     if world == 1 and not args.no_cpu_baseline:
         from oracle import linear as lo
