@@ -271,6 +271,24 @@ def test_small_call_path_ragged(dy, orc, seed, L, B, caps):
         check_records(orc, wr, gpu_run(dy, wr), orc.run(wr), where=f"small-replan(seed={seed})")
 
 
+@pytest.mark.parametrize("seed,L,B,caps,nmin,nmax", [(321, 2, 2, True, 9, 12), (322, 8, 3, False, 13, 16), (323, 3, 8, True, 9, 16)])
+def test_small_call_path_many_nodes(dy, orc, seed, L, B, caps, nmin, nmax):
+    # 9 to 16 nodes of one or two options: still at most 2^16 plans, so k_small takes them -- through the instantiations
+    # of its walk that bound the node count by 12 and 16 (the ragged test above stops at 8 nodes)
+    w = wl.random_workload(seed, R=20, nmin=nmin, nmax=nmax, kmin=1, kmax=2, B=B, M=3, L=L, caps=caps, tool_p=0.05, edge_p=0.3)
+    g = gpu_run(dy, w)
+    st = dy[1].dyplan_last_stats()
+    check_records(orc, w, g, orc.run(w), where=f"small-many-nodes(seed={seed})")
+    binding, ctx = dy
+    import torch
+    dw = binding.upload(w)
+    binding.launch(ctx, dw)
+    torch.cuda.synchronize()
+    assert ctx.dyplan_last_stats()["small_requests"] == int((orc.run(w)["status"].reshape(-1, L)[:, 0] != 2).sum())
+    wr = wl.random_replan_workload(seed + 50, R=20, nmin=nmin, nmax=nmax, kmin=1, kmax=3, B=B, M=3, caps=caps, flags=wl.FLAG_FIXED_IN_PLACE)
+    check_records(orc, wr, gpu_run(dy, wr), orc.run(wr), where=f"small-many-nodes-replan(seed={seed})")
+
+
 # ---- scorer classes: fp32 slack DP for small exact ranges, int32 slack DP for the rest ----------------
 def gpu_run_stats(dy, w):
     g = gpu_run(dy, w)
