@@ -240,8 +240,10 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   // persistent grids: every block resident, work pulled from device counters
   const int grid = ctx->sm_count * occ;
   const int fgrid = ctx->sm_count * focc;
-  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * kFastItemsPerWarp;
-  const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * (target_items_f > 32768u ? target_items_f : 32768u);
+  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * fast_items_per_warp(focc);
+  // room for 4x the items aimed at: k_plan cuts the last eighth of the requests into 4x smaller items (a short tail:
+  // 1.4x the items when the requests are alike, more when the last ones are the large ones) and checks the exact count
+  const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * (4u * target_items_f > 32768u ? 4u * target_items_f : 32768u);
   if ((rc = ensure(ctx, ctx->blob, R * blob_stride_words(L) * 4))) return rc;
   if ((rc = ensure(ctx, ctx->item_off, 2 * (R + 1) * 4))) return rc;
   if ((rc = ensure(ctx, ctx->done, R * 4))) return rc;
@@ -882,7 +884,7 @@ extern "C" int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, in
   }
   const int grid = ctx->sm_count * occ;
   const int fgrid = ctx->sm_count * focc;
-  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * kFastItemsPerWarp;
+  const uint32_t target_items_f = (uint32_t)(fgrid * kFastWarps) * fast_items_per_warp(focc);
   const uint32_t max_items = (uint32_t)(2 * R + 2) + 2u * kStaticItemsPerClass;
 
   CallArgs a;

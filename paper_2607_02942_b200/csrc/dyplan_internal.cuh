@@ -31,7 +31,11 @@ constexpr int kSmallBlocksPerSm = SMALL_BPS;   // blocks of k_small per SM that 
 constexpr unsigned long long kSmallMaxEvals = 1ull << 21;   // (plan, level) evaluations of a request k_small takes
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
-constexpr uint32_t kFastItemsPerWarp = 12;   // work items to aim for per resident warp (measured: 8 and 24 lose 4-7 % on cfg4)
+// work items to aim for per resident warp of k_fscore.  Measured on configs[1..4] (kernel ms): with 4 blocks per SM
+// (L <= 4) 8 / 10 / 12 / 16 items give 2.555 / 2.532 / 2.566 / 2.699 on configs[1]; with 3 blocks per SM (L >= 6)
+// 8 / 10 / 12 / 16 / 24 give 52.0 / 49.4 / 48.8 / 49.6 / 51.0 on configs[4]: about 36-40 items per scheduler either way
+// (fewer: a longer tail; more: the per-item prologue, ticket and fence)
+__host__ __device__ inline uint32_t fast_items_per_warp(int blocks_per_sm) { return blocks_per_sm >= 4 ? 10u : 12u; }
 constexpr float kBigF = 1099511627776.0f; // 2^40: above every slack, latency and demand the ABI admits (< 2^31)
 // fast class: outer indices per work item of a request whose node 2 has K2 options -- the call-wide figure rounded up
 // so that each of the 32 lanes gets a whole number of node-2 sweeps (no idle-lane tail inside full items)

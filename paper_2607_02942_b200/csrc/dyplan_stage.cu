@@ -617,22 +617,31 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   pif = ((pif + 31) / 32) * 32;
   if (pif < 32) pif = 32;
   const bool small_f = total_f / warps < 1024;   // not enough outer indices for one lane-aligned item per resident warp
-  // the last eighth of the requests is cut into 4x smaller items: items are handed out in request order, so the warps
-  // finish within a quarter of an item of each other (measured with 12 items per warp: 1 % on cfg1, 1.5 % on cfg4)
-  uint32_t tail_start = 0xffffffffu;
-  if (!small_f && R >= 2 && pif >= 4 * need && pif >= 4 * 256) tail_start = (uint32_t)(R - (R / 8 > 0 ? R / 8 : 1));
-  uint32_t cw = 0, cf = 0;
-  for (long long r = r0; r < r1; r++) {
-    const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
-    if (h->status != DYPLAN_ST_OK || h->klass == kClassSmall) continue;
-    if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_f); cf += (uint32_t)((h->outer_total + q - 1) / q); }
-    else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
+  // A short tail: items are handed out in request order, so the last sixteenth of the requests is cut into 4x smaller
+  // items and the warps finish within one small item of each other (measured per-warp exit times on configs[1]: with
+  // equal items the warps idled 5.6 % of the launch at its end; last 1/4, 1/8, 1/16, 1/32 of the requests cut: 2.635 /
+  // 2.589 / 2.566 / 2.563 ms; a second level of 16x smaller items lost more to the per-item prologue than it gained).
+  // The exact item count decides whether the cut fits the records' buffer.
+  int tail_mode = (!small_f && R >= 2 && pif >= 4 * 256) ? 1 : 0;
+  uint32_t tail_start, runw, runf, total_items_w, total_items_f;
+  for (;;) {
+    tail_start = tail_mode >= 1 ? (uint32_t)(R - (R / 16 > 0 ? R / 16 : 1)) : 0xffffffffu;
+    uint32_t cw = 0, cf = 0;
+    for (long long r = r0; r < r1; r++) {
+      const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
+      if (h->status != DYPLAN_ST_OK || h->klass == kClassSmall) continue;
+      if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_f); cf += (uint32_t)((h->outer_total + q - 1) / q); }
+      else cw += (uint32_t)((h->outer_total + pio - 1) / pio);
+    }
+    runw = block_exclusive_scan_1024(s_cnt, tid, cw);
+    total_items_w = s_cnt[1023];
+    __syncthreads();
+    runf = block_exclusive_scan_1024(s_cnt, tid, cf);
+    total_items_f = s_cnt[1023];
+    __syncthreads();
+    if (tail_mode == 0 || (unsigned long long)total_items_w + total_items_f <= (unsigned long long)a.max_items) break;   // block-uniform
+    tail_mode--;
   }
-  uint32_t runw = block_exclusive_scan_1024(s_cnt, tid, cw);
-  const uint32_t total_items_w = s_cnt[1023];
-  __syncthreads();
-  uint32_t runf = block_exclusive_scan_1024(s_cnt, tid, cf);
-  const uint32_t total_items_f = s_cnt[1023];
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     a.item_off[r] = runw;
