@@ -645,6 +645,35 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (last) {
       // ---- last warp of this request: reduce its items' records and emit the bundle (fused K_final) ----
       __threadfence();
+      if constexpr (L >= 6) {
+        // many levels: a lane takes an item and reads the records of all its levels (contiguous: one line for 8 levels,
+        // the loads independent), keeping a best per level -- level by level, every line is fetched Lr times with one
+        // load in flight, 0.4 ms for the 5 K items of configs[4]'s last request, at the very end of the launch
+        Best v[L];
+#pragma unroll
+        for (int l = 0; l < L; l++) { v[l].C = -1.0f; v[l].T = INT32_MAX; v[l].idx = kNoIdx; }
+        for (uint32_t j = lane; j < n_it; j += 32) {
+          const float4* pp = (const float4*)&a.partial[(size_t)(rec_base + first_item + j) * Lr];
+          float4 raw[L];
+#pragma unroll
+          for (int l = 0; l < L; l++) if (l < Lr) raw[l] = __ldcg(pp + l);
+#pragma unroll
+          for (int l = 0; l < L; l++) {
+            if (l < Lr) {
+              Best o; o.C = raw[l].x; o.T = __float_as_int(raw[l].y);
+              o.idx = ((unsigned long long)__float_as_uint(raw[l].w) << 32) | (unsigned long long)__float_as_uint(raw[l].z);
+              if (better(o.C, o.T, o.idx, v[l])) v[l] = o;
+            }
+          }
+        }
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+          if (l < Lr) {
+            const Best w = warp_best(v[l]);
+            if (lane == l) mine = w;
+          }
+        }
+      } else
       for (int l = 0; l < Lr; l++) {
         Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
         for (uint32_t j = lane; j < n_it; j += 32) {
