@@ -534,6 +534,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
   const unsigned long long pif = a.st->per_item_outer_f;
   const bool small_call = a.st->small_call_f != 0;
   const uint32_t tail_start = a.st->tail_start_f;
+  const uint32_t perm_nA = a.st->perm_nA, perm_sA = a.st->perm_sA, perm_sB = a.st->perm_sB;
   if (lane == 0) mbar_init(&ws->bar, 1);
   __syncwarp();
   uint32_t phase = 0;
@@ -545,6 +546,9 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (lane == 0) item = atomicAdd(&a.st->next_item_f, 1u);
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= total_items) break;
+    // hand-out order: strided over the regular items, then over the tail's small ones (CallState.perm_*)
+    item = item < perm_nA ? (uint32_t)(((unsigned long long)item * perm_sA) % perm_nA)
+                          : perm_nA + (uint32_t)(((unsigned long long)(item - perm_nA) * perm_sB) % (total_items - perm_nA));
     long long r;
     {   // largest r with item_off_f[r] <= item (every lane searches: uniform, L2-resident)
       long long lo = 0, hi = a.in.R;

@@ -112,6 +112,11 @@ struct CallState {
   uint32_t approx_requests;         // fast class: requests verified in int32 (ReqHdr.approx)
   uint32_t small_requests;          // requests solved by k_small
   uint32_t pad0;
+  // fast class: the order in which work items are handed out.  Items are numbered request by request; the t-th item
+  // handed out is item (t * perm_sA) mod perm_nA among the first perm_nA (the regular items), then the same with perm_sB
+  // among the rest (the small items of the tail); the strides are coprime to the counts and a little above the items of
+  // one request, so consecutive hand-outs fall on consecutive requests and every request is visited all along the launch
+  uint32_t perm_nA, perm_sA, perm_sB, pad2;
 };
 // outer indices per item of request r before rounding (k_plan and k_fscore must agree)
 __host__ __device__ inline unsigned long long fast_pif_of(unsigned long long pif, uint32_t tail_start, long long r) {

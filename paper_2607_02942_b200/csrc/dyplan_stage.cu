@@ -560,6 +560,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
         st->slow_steps = 0; st->bound_skipped = 0;
         st->total_items = 0; st->next_item = 0; st->total_items_f = 0; st->next_item_f = 0;
         st->fast_requests = 0; st->small_call_f = 1u; st->tail_start_f = 0xffffffffu; st->approx_requests = 0; st->small_requests = is_small; st->pad0 = 0;
+        st->perm_nA = 0; st->perm_sA = 1; st->perm_sB = 1; st->pad2 = 0;
       }
       return;
     }
@@ -642,18 +643,46 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
     if (tail_mode == 0 || (unsigned long long)total_items_w + total_items_f <= (unsigned long long)a.max_items) break;   // block-uniform
     tail_mode--;
   }
+  __shared__ uint32_t s_nA;
+  if (tid == 0) s_nA = total_items_f;   // (no tail: every item is a regular one)
+  __syncthreads();
   for (long long r = r0; r < r1; r++) {
     const ReqHdr* h = (const ReqHdr*)(a.blob + (size_t)r * blob_stride);
     a.item_off[r] = runw;
     a.item_off_f[r] = runf;
+    if ((unsigned long long)r == tail_start) s_nA = runf;
     if (h->status != DYPLAN_ST_OK || h->klass == kClassSmall) continue;
     if (h->klass == kClassFast) { const unsigned long long q = fast_item_outer(fast_pif_of(pif, tail_start, r), h->Kp[2], small_f); runf += (uint32_t)((h->outer_total + q - 1) / q); }
     else runw += (uint32_t)((h->outer_total + pio - 1) / pio);
   }
+  __syncthreads();
   if (tid == 1023) {
     a.item_off[R] = total_items_w;
     a.item_off_f[R] = total_items_f;
     CallState* st = a.st;
+    // Hand-out order of the fast items (CallState.perm_*).  Handed out request by request, all items of a request would
+    // start within microseconds of each other, each with nothing better than k_seed's threshold, and each would climb
+    // to the optimum on its own through the slow path (measured: about 27 us per item on configs[1], a tenth of the
+    // launch).  Strided, a request's items are spread over the whole launch and start from what the earlier ones published.
+    {
+      const uint32_t nA = s_nA, nB = total_items_f - s_nA;
+      const uint32_t reqs = n_fast ? n_fast : 1u;
+      auto stride_for = [](uint32_t n, uint32_t per_request) -> uint32_t {
+        if (n <= 2) return 1u;
+        uint32_t s = per_request + 1u;
+        if (s >= n) s = 1u;
+        for (;; s++) {
+          if (s >= n) s = 1u;
+          uint32_t x = n, y = s;
+          while (y) { const uint32_t t = x % y; x = y; y = t; }
+          if (x == 1u) return s;
+        }
+      };
+      st->perm_nA = nA;
+      st->perm_sA = stride_for(nA, (nA + reqs - 1) / reqs);
+      st->perm_sB = stride_for(nB, (uint32_t)((4ull * nB + reqs - 1) / reqs));   // (a sixteenth of the requests, 4x the items each: roughly)
+      st->pad2 = 0;
+    }
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
     st->slow_steps = 0; st->bound_skipped = 0;
     st->total_items = total_items_w; st->next_item = 0; st->total_items_f = total_items_f; st->next_item_f = 0;
