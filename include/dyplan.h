@@ -20,7 +20,8 @@
  *   field is a DEVICE pointer on the ctx's device; in the *_host calls every pointer field is a HOST pointer
  *   (the library stages the copies itself, on `stream`, and returns after the results are in the host buffers).
  *   The caller owns every buffer and keeps it alive until the stream work completes.  The library allocates only
- *   its own scratch inside dyplan_ctx (grown on demand; growing calls cudaMalloc, nothing else synchronises).
+ *   its own scratch inside dyplan_ctx (grown on demand; growing calls cudaMalloc, nothing else synchronises; the
+ *   *_host calls also keep a 256 KB pinned staging buffer there).  dyplan_compile_static allocates nothing at all.
  * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Plain calls are
  *   asynchronous on it.  A ctx owns one set of scratch: a call issued on another stream than the previous call of the
  *   same ctx first waits, on the device, for that call's work (an event; the host does not block), so calls of one ctx
@@ -257,7 +258,11 @@ DYPLAN_API int dyplan_compile_linear(dyplan_ctx* ctx, const dyplan_batch* in, co
 /* The compile / replan / select / compile_linear calls with HOST pointers everywhere (batch fields, multipliers, masks,
  * cost, outputs, extras).  The library copies
  * inputs to the device, runs the same kernels and copies the results back, all on `stream`, and returns after a
- * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied. */
+ * stream synchronise.  h2d_bytes / d2h_bytes (optional) receive the bytes copied.  Calls below 256 KB move through ONE
+ * pinned staging buffer owned by the ctx (one copy each way); a compile / replan call whose packed inputs are at most
+ * 8 KB -- one admission-time request -- does not use the copy engine at all: the staging kernel fetches the inputs from
+ * the pinned buffer itself and the records are stored straight into it (pinned memory is device-visible), so the call is
+ * two launches and a synchronise.  The bytes reported are the same either way. */
 DYPLAN_API int dyplan_compile_host(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const int32_t* mult_pm, dyplan_bundle* out,
                         void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 DYPLAN_API int dyplan_replan_host(dyplan_ctx* ctx, const dyplan_batch* in, const uint32_t* dispatched_mask,

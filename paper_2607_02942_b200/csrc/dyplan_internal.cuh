@@ -24,10 +24,7 @@ constexpr int kClassFast = 1;        // fp32 slack DP (k_fscore): exact when eve
 constexpr int kClassSmall = 2;       // a small request of a small call: int32 layout, solved by k_small (dyplan_small.cu)
 constexpr int kSmallMaxR = 32;       // calls of at most this many requests try the small path
 constexpr int kSmallThreads = 128;
-#ifndef SMALL_BPS
-#define SMALL_BPS 4
-#endif
-constexpr int kSmallBlocksPerSm = SMALL_BPS;   // blocks of k_small per SM that the requests of a call share
+constexpr int kSmallBlocksPerSm = 4;   // blocks of k_small per SM that the requests of a call share (2, 3, 4, 6, 8, 12 measured on configs[0]: 70 / 64 / 60 / 62 / 65 / 67 us)
 constexpr unsigned long long kSmallMaxEvals = 1ull << 21;   // (plan, level) evaluations of a request k_small takes
 constexpr int kFastBlobWords = 1536; // per-warp shared-memory window of k_fscore (6 KB)
 constexpr int kFastWarps = 4;        // warps per k_fscore block (each warp works on its own item)
