@@ -21,6 +21,9 @@ namespace dyplan {
 #ifndef CTX_SHARED_MIN_L
 #define CTX_SHARED_MIN_L 4
 #endif
+#ifndef FIN_MIN_L
+#define FIN_MIN_L 6
+#endif
 template <int L>
 struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
@@ -649,7 +652,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (last) {
       // ---- last warp of this request: reduce its items' records and emit the bundle (fused K_final) ----
       __threadfence();
-      if constexpr (L >= 6) {
+      if constexpr (L >= FIN_MIN_L) {
         // many levels: a lane takes an item and reads the records of all its levels (contiguous: one line for 8 levels,
         // the loads independent), keeping a best per level -- level by level, every line is fetched Lr times with one
         // load in flight, 0.4 ms for the 5 K items of configs[4]'s last request, at the very end of the launch

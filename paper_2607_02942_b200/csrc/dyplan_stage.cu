@@ -441,7 +441,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
 // the last node down) and publish the best feasible C per level.  A threshold is only ever the C32 of a plan that
 // exists and is feasible, so the enumeration still meets that plan (ties pass the screen) and the result does not
 // depend on the seeds. ----
-constexpr int kSeedThreads = 128, kSeedsPerThread = 4;
+constexpr int kSeedThreads = 128, kSeedsPerThread = 2;   // random plans per thread (plus one plan of the trade-off family)
 __global__ void __launch_bounds__(kSeedThreads) k_seed(CallArgs a) {
   __shared__ __align__(16) uint32_t sb[kFastBlobWords];
   const long long r = blockIdx.x;
@@ -465,7 +465,14 @@ __global__ void __launch_bounds__(kSeedThreads) k_seed(CallArgs a) {
   const int* p_idem = p_ilat + nsp * Lp;
   const int slo_c = sh->slo_c;
   int su[16][DYPLAN_MAX_LEVELS];
-  for (int sidx = 0; sidx < kSeedsPerThread; sidx++) {
+  // Seeds: kSeedsPerThread random plans per thread, then one plan of a one-parameter family that follows the trade-off
+  // the method is about -- per node the option with the largest factor among those whose duration (at one level, the
+  // thread's) is at most theta times the node's longest, theta = 1/32 .. 1 over the threads.  Random plans give a
+  // threshold near the top 0.2 % of the space; a call of one or two mid-size requests then spent its time in slow-path
+  // re-walks while every warp climbed from there on its own (configs[1], one request: 5931 re-walks, 0.20 ms).
+  const int fam_theta = (tid & 31) + 1, fam_level = (tid >> 5) % (L > 0 ? L : 1);
+  for (int sidx = 0; sidx <= kSeedsPerThread; sidx++) {
+    const bool family = sidx == kSeedsPerThread;
     uint32_t x = (uint32_t)r * 0x9E3779B9u + (uint32_t)(sidx * kSeedThreads + tid) * 0x85EBCA6Bu + 0x27D4EB2Fu;
     float C = 1.0f;
     int D[8], ms[DYPLAN_MAX_LEVELS];
@@ -476,7 +483,24 @@ __global__ void __launch_bounds__(kSeedThreads) k_seed(CallArgs a) {
     for (int i = Np - 1; i >= 0; --i) {
       x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;   // integer hash, one draw per node
       const int kp = i == 0 ? K0p : sh->Kp[i];
-      const int slot = sh->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
+      int slot = sh->optbase[i] + (int)((x >> 8) % (uint32_t)kp);
+      if (family) {
+        const int ob = sh->optbase[i];
+        long long dmax = 0;
+        for (int k = 0; k < kp; k++) {
+          if (!(p_f[ob + k] > 0.0f)) continue;   // padding slot
+          const long long d = approx ? (long long)p_ilat[(ob + k) * Lp + fam_level] : (long long)(-p_nlat[(ob + k) * Lp + fam_level]);
+          dmax = d > dmax ? d : dmax;
+        }
+        const long long lim = dmax * fam_theta / 32;
+        float bf = -1.0f; long long bd = 0;
+        for (int k = 0; k < kp; k++) {
+          const float f = p_f[ob + k];
+          if (!(f > 0.0f)) continue;
+          const long long d = approx ? (long long)p_ilat[(ob + k) * Lp + fam_level] : (long long)(-p_nlat[(ob + k) * Lp + fam_level]);
+          if (d <= lim ? (bf < 0.0f || bd > lim || f > bf || (f == bf && d < bd)) : (bf < 0.0f || (bd > lim && d < bd))) { bf = f; bd = d; slot = ob + k; }
+        }
+      }
       C *= p_f[slot];
       const int be = p_be[slot] & 7;
       const int dm = approx ? p_idem[slot] : (int)p_dem[slot];
