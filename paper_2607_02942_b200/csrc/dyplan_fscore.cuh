@@ -21,9 +21,6 @@ namespace dyplan {
 #ifndef CTX_SHARED_MIN_L
 #define CTX_SHARED_MIN_L 4
 #endif
-#ifndef FIN_MIN_L
-#define FIN_MIN_L 6
-#endif
 template <int L>
 struct __align__(16) FWarpShared {
   uint32_t blob[kFastBlobWords];   // the request's staged blob (1-D TMA bulk copy)
@@ -652,7 +649,7 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
     if (last) {
       // ---- last warp of this request: reduce its items' records and emit the bundle (fused K_final) ----
       __threadfence();
-      if constexpr (L >= FIN_MIN_L) {
+      if constexpr (L >= 6) {
         // many levels: a lane takes an item and reads the records of all its levels (contiguous: one line for 8 levels,
         // the loads independent), keeping a best per level -- level by level, every line is fetched Lr times with one
         // load in flight, 0.4 ms for the 5 K items of configs[4]'s last request, at the very end of the launch
@@ -683,12 +680,22 @@ __global__ void __launch_bounds__(kFastWarps * 32, (L >= 6 ? 3 : 4)) k_fscore(co
       } else
       for (int l = 0; l < Lr; l++) {
         Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
-        for (uint32_t j = lane; j < n_it; j += 32) {
-          const Partial* pp = &a.partial[(size_t)(rec_base + first_item + j) * Lr + l];
-          const float4 raw = __ldcg((const float4*)pp);
-          Best o; o.C = raw.x; o.T = __float_as_int(raw.y);
-          o.idx = ((unsigned long long)__float_as_uint(raw.w) << 32) | (unsigned long long)__float_as_uint(raw.z);
-          if (better(o.C, o.T, o.idx, v)) v = o;
+        // (four loads in flight: a request of a small call is cut into a thousand items and more, and this walk by its
+        // last warp, one load at a time, was half of such a call's scoring time)
+        for (uint32_t j0 = lane; j0 < n_it; j0 += 128) {
+          float4 raw[4];
+#pragma unroll
+          for (int q = 0; q < 4; q++) {
+            const uint32_t j = j0 + 32u * q;
+            raw[q] = j < n_it ? __ldcg((const float4*)&a.partial[(size_t)(rec_base + first_item + j) * Lr + l])
+                              : make_float4(-1.0f, __int_as_float(INT32_MAX), __uint_as_float(0xffffffffu), __uint_as_float(0xffffffffu));
+          }
+#pragma unroll
+          for (int q = 0; q < 4; q++) {
+            Best o; o.C = raw[q].x; o.T = __float_as_int(raw[q].y);
+            o.idx = ((unsigned long long)__float_as_uint(raw[q].w) << 32) | (unsigned long long)__float_as_uint(raw[q].z);
+            if (better(o.C, o.T, o.idx, v)) v = o;
+          }
         }
         v = warp_best(v);
         if (lane == l) mine = v;
