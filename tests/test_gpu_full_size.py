@@ -7,7 +7,8 @@ default context), checked on what the oracle can afford:
   * cfg4 (2.18e9 plans per request): requests 0 and 1 against the brute-force oracle's stored records
     (tests/golden/cfg4_requests_0_1_oracle.txt, written by tests/golden/make_cfg4_oracle_golden.py from oracle/ alone),
     all matching rules; every one of the 128 records against the independent MILP of PIN13 (HiGHS);
-  * cfg3's queries once more with non-prefix (down-set) dispatched sets, both replan semantics.
+  * cfg3's queries once more with non-prefix (down-set) dispatched sets, both replan semantics;
+  * cfg1 once more with every duration x 3000 (the approx class of the fp32 scorer), same checks.
 """
 from __future__ import annotations
 
@@ -92,6 +93,25 @@ def test_cfg1_full(dy, orc):
     assert check_own_plan(orc, w, g, range(256 * 4)) > 900
     c = check_sampled_requests(orc, w, g, [0, 101, 255], "cfg1-full")
     assert c["records"] == 12
+
+
+def test_cfg1_full_with_second_scale_latencies(dy, orc):
+    # configs[1] with every duration and SLO x 3000 (seconds to minutes): the requests leave the fp32
+    # scorer's exact range and run on its verified instantiation (conservative fp32 screen, int32 check of every
+    # candidate) -- at full size, in the launch configuration bench.py times for its x 3000 leg
+    w = wl.make_config(1)
+    w.batch.lat_us = (w.batch.lat_us.astype(np.int64) * 3000).astype(np.int32)
+    w.batch.slo_us = (w.batch.slo_us.astype(np.int64) * 3000).astype(np.int32)
+    g, st = gpu_run(dy, w)
+    assert st["fast_requests"] == 256 and st["approx_requests"] == 256
+    assert check_own_plan(orc, w, g, range(256 * 4)) > 900
+    c = check_sampled_requests(orc, w, g, [0, 101, 255], "cfg1-full-x3000")
+    assert c["records"] == 12
+    # scaling every duration and the SLO by the same factor scales T and leaves the optimum's plan alone
+    # (floor(tau * 3000 * m / 1000) = 3 * tau * m exactly, and floor(tau * m / 1000) * 3000 <= it: the feasible set can
+    # only shrink by plans within one microsecond-rounding of the SLO), so most records keep their plan
+    g1, _ = gpu_run(dy, wl.make_config(1))
+    assert (g1["plan_idx"] == g["plan_idx"]).mean() > 0.9
 
 
 def test_cfg2_full(dy, orc):
