@@ -256,7 +256,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.in = *in; a.out = *out; a.L = L; a.mult = mult; a.dispatched = dispatched; a.fixed_choice = fixed_choice;
   a.flags = flags; a.is_replan = is_replan ? 1 : 0; a.ctx_flags = ctx->flags;
   a.blob = (uint32_t*)ctx->blob.p; a.item_off = (uint32_t*)ctx->item_off.p; a.item_off_f = a.item_off + (R + 1);
-  a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f;
+  a.done = (uint32_t*)ctx->done.p; a.target_items_f = target_items_f; a.fast_warps = (uint32_t)(fgrid * kFastWarps);
   a.gthr = (float*)ctx->gthr.p; a.partial = (Partial*)ctx->partial.p; a.st = (CallState*)ctx->state.p;
   a.max_items = max_items;
   a.img_src = (const uint4*)img_src; a.img_dst = (uint4*)img_dst; a.img_vec = (uint32_t)((img_bytes + 15) / 16);
@@ -901,7 +901,7 @@ extern "C" int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, in
   const size_t small_recs = a.small_mode ? R * (size_t)a.small_split : 0;
   a.partial = sc.take<Partial>((small_recs > max_items ? small_recs : (size_t)max_items) * L);
   a.st = sc.take<CallState>(1);
-  a.target_items_f = target_items_f;
+  a.target_items_f = target_items_f; a.fast_warps = (uint32_t)(fgrid * kFastWarps);
   a.max_items = max_items;
   if (sc.off > (size_t)DYPLAN_STATIC_SCRATCH_BYTES) {   // (cannot happen within the limits above: a guard for a device with > 1000 SMs)
     snprintf(ctx->errbuf, sizeof(ctx->errbuf), "dyplan_compile_static: the scratch layout needs %zu bytes, the static array holds %u",

@@ -145,6 +145,7 @@ struct CallArgs {                   // passed by value to the kernels
   CallState* st;
   uint32_t max_items;               // bound on wide items + fast items
   uint32_t target_items_f;          // fast class: work items to aim for (a multiple of the resident warps)
+  uint32_t fast_warps;              // fast class: resident warps of k_fscore's persistent grid
 };
 
 

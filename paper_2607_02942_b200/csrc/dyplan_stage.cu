@@ -634,8 +634,8 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
   need = (total_f + budget - 1) / budget;
   if (need > pif) pif = need;
   // small calls: an item should carry at least 8 outer indices per lane (its fixed cost is a few thousand instructions)
-  // unless that would leave resident warps without work (target_items_f = 24 items per resident warp)
-  const unsigned long long warps = a.target_items_f / 16 ? a.target_items_f / 16 : 1;
+  // unless that would leave resident warps without work
+  const unsigned long long warps = a.fast_warps ? a.fast_warps : 1;
   unsigned long long floor_f = (total_f + warps - 1) / warps;
   floor_f = floor_f > 256 ? 256 : floor_f;
   if (floor_f > pif) pif = floor_f;
