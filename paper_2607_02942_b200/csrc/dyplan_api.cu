@@ -263,13 +263,24 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
   a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
 
-  // The plain (device-pointer) call cannot see the option counts, but the sizes in the struct bound them: a request's
-  // plan count is at most the product of ALL option counts of the batch, which is at most (KK / NN)^NN (AM-GM; exact
-  // for one request with equal counts).  When that bound times L fits k_small's limit, every request that k_stage
-  // accepts is small, and the batched scorers have nothing to do: their four launches (about 20 us) are not issued.
-  if (a.small_mode && !all_small && in->NN > 0 && in->KK >= in->NN &&
-      (double)in->NN * log2((double)in->KK / (double)in->NN) + log2((double)L) <= 20.99)
-    all_small = true;
+  // The plain (device-pointer) call cannot see the option counts, but the sizes in the struct bound them: a request has
+  // at most min(NN, 16) nodes, at most KK options in all and at most 16 per node, so at most
+  // max_n min(KK / n, 16)^n plans (AM-GM; exact for one request with equal counts).  When that bound times L fits
+  // k_small's limit, every request that k_stage accepts is small, and the batched scorers have nothing to do: their
+  // four launches (about 20 us) are not issued.  (Taking the maximum over n keeps the bound valid when NN overstates
+  // the node count; a KK that understates the option count makes k_stage reject the request.)
+  if (a.small_mode && !all_small && in->NN > 0 && in->KK > 0) {
+    double worst = 0.0;   // log2 of the bound
+    const int nmax = in->NN < DYPLAN_MAX_NODES ? in->NN : DYPLAN_MAX_NODES;
+    for (int n = 1; n <= nmax; n++) {
+      double k = (double)in->KK / (double)n;
+      if (k > (double)DYPLAN_MAX_OPTS) k = (double)DYPLAN_MAX_OPTS;
+      if (k < 1.0) k = 1.0;
+      const double b = (double)n * log2(k);
+      if (b > worst) worst = b;
+    }
+    if (worst + log2((double)L) <= 20.99) all_small = true;
+  }
   CK(launch_stage(a, stream));
   int launches = 1;
   const bool only_small = a.small_mode && all_small;

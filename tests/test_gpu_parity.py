@@ -214,7 +214,7 @@ def test_small_call_path_takes_small_requests_only(dy, orc):
     import torch
     binding, ctx = dy
     # configs[0] alone: one launch pair (stage + small) through the host entry point, and through the device one too:
-    # the sizes in the struct bound the plan count ((KK / NN)^NN x L = 8^6 x 3 <= 2^21), so the batched scorers are not launched
+    # the sizes in the struct bound the plan count (max_n min(KK / n, 16)^n x L = 8^6 x 3 <= 2^21), so the batched scorers are not launched
     w = wl.make_config(0)
     dw = binding.upload(w)
     binding.launch(ctx, dw)
@@ -222,7 +222,7 @@ def test_small_call_path_takes_small_requests_only(dy, orc):
     st = ctx.dyplan_last_stats()
     assert st["small_requests"] == 1 and st["fast_requests"] == 0 and st["plans"] == w.n_plans_total() and st["launches"] == 2
     check_records(orc, w, dw.out.host(), orc.run(w), where="small cfg0")
-    # the same shape with 8 levels: (KK / NN)^NN x L = 2^21 exactly, which 20.99 bits do not cover -- the device call then
+    # the same shape with 8 levels: the bound x L = 2^21 exactly, which 20.99 bits do not cover -- the device call then
     # launches all six kernels although k_stage finds the request small (the bound is deliberately on the safe side)
     w8 = wl.random_workload(302, R=1, nmin=6, nmax=6, kmin=8, kmax=8, B=2, M=2, L=8, caps=False, tool_p=0.0)
     dw8 = binding.upload(w8)
