@@ -323,7 +323,9 @@ DYPLAN_API int dyplan_measure_issue_rates(dyplan_ctx* ctx, dyplan_issue_rate* ou
  * and it keeps the previous call's contents (the kernels reset the counters they need at the start of each call, as
  * they do for the ctx's scratch).  Two calls that OVERLAP on the GPU (different streams, different ctxs, different
  * host threads) RACE on it and give garbage: issue them on one stream, or order them with events.  The library adds no
- * ordering of its own here.  dyplan_last_stats after this call reports `launches` and `sm_count` only. */
+ * ordering of its own here.  dyplan_last_stats after this call reports `launches` and `sm_count` only.
+ * Graph capture: after one call outside capture on the device (it looks up the array's address and the kernels'
+ * occupancy), the call only enqueues kernel launches on `stream` and can be captured and replayed. */
 #define DYPLAN_STATIC_MAX_REQUESTS 512
 #define DYPLAN_STATIC_SCRATCH_BYTES (16u << 20)
 #define DYPLAN_ERR_STATIC_LIMIT (-5) /* the call does not fit the static scratch of dyplan_compile_static */

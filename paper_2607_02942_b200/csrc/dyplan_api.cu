@@ -201,6 +201,26 @@ static int check_bundle(const dyplan_bundle* o) {
   return DYPLAN_OK;
 }
 
+// The plain (device-pointer) calls cannot see the option counts, but the sizes in the struct bound them: a request has
+// at most min(NN, 16) nodes, at most KK options in all and at most 16 per node, so at most max_n min(KK / n, 16)^n plans
+// (AM-GM; exact for one request with equal counts).  When that bound times L fits k_small's limit, every request that
+// k_stage accepts is small, and the batched scorers have nothing to do: their four launches (about 20 us) are not
+// issued.  (Taking the maximum over n keeps the bound valid when NN overstates the node count; a KK that understates
+// the option count makes k_stage reject the request.)
+static bool sizes_prove_all_small(const dyplan_batch* in, int32_t L) {
+  if (in->NN <= 0 || in->KK <= 0) return false;
+  double worst = 0.0;   // log2 of the bound
+  const int nmax = in->NN < DYPLAN_MAX_NODES ? in->NN : DYPLAN_MAX_NODES;
+  for (int n = 1; n <= nmax; n++) {
+    double k = (double)in->KK / (double)n;
+    if (k > (double)DYPLAN_MAX_OPTS) k = (double)DYPLAN_MAX_OPTS;
+    if (k < 1.0) k = 1.0;
+    const double b = (double)n * log2(k);
+    if (b > worst) worst = b;
+  }
+  return worst + log2((double)L) <= 20.99;
+}
+
 // compile and replan share everything but two arguments
 // all_small: the caller (a *_host entry point, which sees the option counts) has established that every request of the
 // call is one k_small takes, so the batched scorers are not launched at all
@@ -263,24 +283,7 @@ static int run_solve(dyplan_ctx* ctx, const dyplan_batch* in, int32_t L, const i
   a.small_mode = (in->R <= kSmallMaxR && !(ctx->flags & DYPLAN_NO_SMALL_PATH)) ? 1 : 0;
   a.small_split = a.small_mode ? (kSmallBlocksPerSm * ctx->sm_count / (int)in->R > 1 ? kSmallBlocksPerSm * ctx->sm_count / (int)in->R : 1) : 1;
 
-  // The plain (device-pointer) call cannot see the option counts, but the sizes in the struct bound them: a request has
-  // at most min(NN, 16) nodes, at most KK options in all and at most 16 per node, so at most
-  // max_n min(KK / n, 16)^n plans (AM-GM; exact for one request with equal counts).  When that bound times L fits
-  // k_small's limit, every request that k_stage accepts is small, and the batched scorers have nothing to do: their
-  // four launches (about 20 us) are not issued.  (Taking the maximum over n keeps the bound valid when NN overstates
-  // the node count; a KK that understates the option count makes k_stage reject the request.)
-  if (a.small_mode && !all_small && in->NN > 0 && in->KK > 0) {
-    double worst = 0.0;   // log2 of the bound
-    const int nmax = in->NN < DYPLAN_MAX_NODES ? in->NN : DYPLAN_MAX_NODES;
-    for (int n = 1; n <= nmax; n++) {
-      double k = (double)in->KK / (double)n;
-      if (k > (double)DYPLAN_MAX_OPTS) k = (double)DYPLAN_MAX_OPTS;
-      if (k < 1.0) k = 1.0;
-      const double b = (double)n * log2(k);
-      if (b > worst) worst = b;
-    }
-    if (worst + log2((double)L) <= 20.99) all_small = true;
-  }
+  if (a.small_mode && !all_small && sizes_prove_all_small(in, L)) all_small = true;
   CK(launch_stage(a, stream));
   int launches = 1;
   const bool only_small = a.small_mode && all_small;
@@ -923,10 +926,13 @@ extern "C" int dyplan_compile_static(dyplan_ctx* ctx, const dyplan_batch* in, in
   CK(launch_stage(a, stream));
   int launches = 1;
   if (a.small_mode) { CK(launch_small(a, stream)); launches++; }
-  CK(launch_seed(a, stream));
-  CK(launch_plan(a, stream));
-  CK(kFLaunch[L - 1](a, fgrid, stream));
-  CK(kLaunch[L - 1](a, nbc, grid, stream));
-  ctx->last_launches = launches + 4;
+  if (!(a.small_mode && sizes_prove_all_small(in, L))) {
+    CK(launch_seed(a, stream));
+    CK(launch_plan(a, stream));
+    CK(kFLaunch[L - 1](a, fgrid, stream));
+    CK(kLaunch[L - 1](a, nbc, grid, stream));
+    launches += 4;
+  }
+  ctx->last_launches = launches;
   return DYPLAN_OK;
 }

@@ -124,3 +124,27 @@ def test_static_scratch_call_allocates_no_device_memory(dy):
         assert_same(w, g, dw.out.host(), "fresh ctx")
     finally:
         ctx.close()
+
+
+def test_static_scratch_call_is_capturable_in_a_cuda_graph(dy):
+    # the reason the entry point exists: nothing in it allocates, synchronises or records an event, so after one warm
+    # call (symbol address, occupancy query, module load) the whole compile is capturable and replays bit for bit
+    import torch
+    binding, ctx = dy
+    for w in (wl.random_workload(seed=9201, R=40, nmin=4, nmax=7, kmin=2, kmax=5, B=3, M=3, L=4), wl.make_config(0)):
+        dw = binding.upload(w, "cuda:0")
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            ctx.dyplan_compile_static(dw.batch, dw.L, dw.mult, dw.out, s)
+        s.synchronize()
+        ref = {k: v.copy() for k, v in dw.out.host().items()}
+        assert_same(w, ref, existing_path(binding, ctx, w), "warm static call")
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ctx.dyplan_compile_static(dw.batch, dw.L, dw.mult, dw.out, s)
+        for _ in range(3):
+            for k in ("plan_idx", "corr", "lat", "status"):
+                dw.out.arrays[k].fill_(0x5A if k == "status" else 77)
+            g.replay()
+            torch.cuda.synchronize()
+            assert_same(w, dw.out.host(), ref, "graph replay")
