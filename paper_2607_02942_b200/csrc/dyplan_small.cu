@@ -18,7 +18,9 @@ namespace dyplan {
 // node; here lane n takes node n -- option counts, the digit of the winner's canonical index, the option's annotations
 // -- so the record costs two round trips to L2 instead of two per node.  C64 is still the product in node order, by
 // one lane, without contraction (definition 4; matches the plain definition bit for bit).
-__device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w) {
+// (ob, K, vn: node `lane`'s first option, option count and vulnerability, fetched by the caller before it reduced the
+// records, so that their round trip is not in front of this one's)
+__device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long long r, int l, const Best& w, int ob, unsigned long long K, float vn) {
   const int lane = threadIdx.x & 31;
   if (w.idx == kNoIdx) {   // warp-uniform
     if (lane == 0) emit_record(a, h, r, l, w);
@@ -28,10 +30,7 @@ __device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long
   const dyplan_bundle& o = a.out;
   const int B = b.B, M = b.M;
   const long long rec = r * a.L + l;
-  const int n0 = h->n0, N = h->n_orig;
-  int ob = 0;
-  unsigned long long K = 1;
-  if (lane < N) { ob = b.opt_off[n0 + lane]; K = (unsigned long long)(b.opt_off[n0 + lane + 1] - ob); }
+  const int N = h->n_orig;
   unsigned long long stride = K;   // inclusive prefix product over the lanes, then shifted: stride of node `lane`
 #pragma unroll
   for (int off = 1; off < 16; off <<= 1) {
@@ -40,13 +39,14 @@ __device__ __noinline__ void emit_small(const CallArgs& a, const ReqHdr* h, long
   }
   stride = __shfl_up_sync(0xffffffffu, stride, 1);
   if (lane == 0) stride = 1;
-  const int k = lane < N ? (int)((w.idx / stride) % K) : 0;
+  int k = 0;
+  if (lane < N) k = ((w.idx | stride) >> 32) == 0 ? (int)(((uint32_t)w.idx / (uint32_t)stride) % (uint32_t)K) : (int)((w.idx / stride) % K);
   double f = 1.0;
   int be = 0, mo = 0, dm = 0;
   if (lane < 16) o.choice[rec * 16 + lane] = lane < N ? (uint8_t)k : (uint8_t)0xFF;
   if (lane < N && !((h->skip_mask >> lane) & 1)) {
     const int op = ob + k;
-    f = __dsub_rn(1.0, __dmul_rn((double)b.vuln[n0 + lane], __dsub_rn(1.0, (double)b.acc[op])));
+    f = __dsub_rn(1.0, __dmul_rn((double)vn, __dsub_rn(1.0, (double)b.acc[op])));
     be = b.backend[op]; mo = b.model[op]; dm = b.demand[op];
   }
   double c = 1.0;
@@ -235,35 +235,35 @@ __global__ void __launch_bounds__(kSmallThreads, 4) k_small(const __grid_constan
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  // ---- last block of this request: the records of all parts, every level (S6).  All 128 threads fetch (the loads of
-  // one thread are independent: four in flight), then warp shuffles, shared memory, and warp l emits level l ----
-#pragma unroll
-  for (int l = 0; l < DYPLAN_MAX_LEVELS; l++) {
-    if (l >= L) break;
+  // ---- last block of this request (S6): warp l takes level l -- the records of all parts with ten loads in flight per
+  // lane (two round trips for 592 parts), shuffles, and the same warp emits; the node constants the emission needs are
+  // fetched first, so their round trip overlaps the records'.  (Measured on configs[0]: this tail was 15 us of the
+  // kernel's 27 when one thread block walked the levels one after the other and the emission fetched on its own.) ----
+  const int n_orig = h->n_orig;
+  int e_ob = 0; unsigned long long e_K = 1; float e_v = 0.0f;
+  if (wid < L && lane < n_orig) {
+    e_ob = a.in.opt_off[h->n0 + lane];
+    e_K = (unsigned long long)(a.in.opt_off[h->n0 + lane + 1] - e_ob);
+    e_v = a.in.vuln[h->n0 + lane];
+  }
+  for (int l = wid; l < L; l += kSmallThreads / 32) {
     Best v; v.C = -1.0f; v.T = INT32_MAX; v.idx = kNoIdx;
-    for (int j0 = tid; j0 < split; j0 += 4 * kSmallThreads) {
-      float4 raw[4];
+    for (int j0 = lane; j0 < split; j0 += 32 * 10) {
+      float4 raw[10];
 #pragma unroll
-      for (int q = 0; q < 4; q++) {
-        const int j = j0 + q * kSmallThreads;
+      for (int q = 0; q < 10; q++) {
+        const int j = j0 + 32 * q;
         raw[q] = j < split ? __ldcg((const float4*)&part_rec[(size_t)j * L + l]) : make_float4(-1.0f, __int_as_float(INT32_MAX), __uint_as_float(0xffffffffu), __uint_as_float(0xffffffffu));
       }
 #pragma unroll
-      for (int q = 0; q < 4; q++) {
+      for (int q = 0; q < 10; q++) {
         Best o; o.C = raw[q].x; o.T = __float_as_int(raw[q].y);
         o.idx = ((unsigned long long)__float_as_uint(raw[q].w) << 32) | (unsigned long long)__float_as_uint(raw[q].z);
         if (better(o.C, o.T, o.idx, v)) v = o;
       }
     }
     v = warp_best(v);
-    if (lane == 0) s_red[l][wid] = v;
-  }
-  __syncthreads();
-  for (int l = wid; l < L; l += kSmallThreads / 32) {
-    Best v = s_red[l][0];
-#pragma unroll
-    for (int w = 1; w < kSmallThreads / 32; w++) { const Best o = s_red[l][w]; if (better(o.C, o.T, o.idx, v)) v = o; }
-    emit_small(a, h, r, l, v);
+    emit_small(a, h, r, l, v, e_ob, e_K, e_v);
   }
   if (tid == 0) { atomicAdd(&a.st->total_plans, (unsigned long long)P); atomicAdd(&a.st->small_requests, 1u); }   // (k_plan sets the totals again when the general scorers run too)
 }
