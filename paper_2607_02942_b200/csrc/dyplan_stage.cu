@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
         if (K[n] < 1 || K[n] > DYPLAN_MAX_OPTS || o0[n] < 0 || o0[n] + K[n] > b.KK) { st = DYPLAN_ST_INVALID; K[n] = 1; }
         else {
           stride[n] = s;
-          if (s > ((1ull << 60) / (unsigned long long)K[n])) st = DYPLAN_ST_TOO_LARGE;
+          if (__umul64hi(s, (unsigned long long)K[n]) != 0ull || s * (unsigned long long)K[n] > (1ull << 60)) st = DYPLAN_ST_TOO_LARGE;   // s K > 2^60, without a division
           s *= (unsigned long long)K[n];
         }
       }
@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
     bool too_large = false;
     for (int i = 0; i < Np; i++) {
       const unsigned long long k = (unsigned long long)__shfl_sync(0xffffffffu, Kp, i);
-      if (P > ((1ull << DYPLAN_MAX_PLANS_LOG2) / k)) too_large = true; else P *= k;
+      if (P * k > (1ull << DYPLAN_MAX_PLANS_LOG2)) too_large = true; else P *= k;   // (P <= 2^40, k <= 16: no overflow; a 64-bit division per node cost this lone warp 2 us)
     }
     if (too_large) {
       if (lane == 0) { h->status = DYPLAN_ST_TOO_LARGE; h->outer_total = 0; h->nslots_pad = 0; h->K0 = 1; h->K1 = 1; }
@@ -369,16 +369,13 @@ __global__ void __launch_bounds__(128) k_stage(CallArgs a) {
       const int ob = __shfl_sync(0xffffffffu, optbase, i), w = __shfl_sync(0xffffffffu, width, i);
       if (s >= ob && s < ob + w) { node = i; k = s - ob; }
     }
-    int ne = -1, nK = 1, no0 = 0, nfix = 0, nfk = 0;
-    uint32_t nkeep = 1u;
-    unsigned long long nstride = 0;
-    for (int i = 0; i < Np; i++) {
-      const int ee = __shfl_sync(0xffffffffu, e, i), kk = __shfl_sync(0xffffffffu, myK, i), oo = __shfl_sync(0xffffffffu, myo0, i);
-      const int ff = __shfl_sync(0xffffffffu, (int)fixed, i), fkk = __shfl_sync(0xffffffffu, fk, i);
-      const uint32_t kp = __shfl_sync(0xffffffffu, keep, i);
-      const unsigned long long ss = __shfl_sync(0xffffffffu, mystride, i);
-      if (i == node) { ne = ee; nK = kk; no0 = oo; nfix = ff; nfk = fkk; nstride = ss; nkeep = kp; }
-    }
+    // the owning node's fields, straight from its lane (a shuffle with a per-lane source)
+    const int src = node < 0 ? 0 : node;
+    int ne = __shfl_sync(0xffffffffu, e, src), nK = __shfl_sync(0xffffffffu, myK, src), no0 = __shfl_sync(0xffffffffu, myo0, src);
+    int nfix = __shfl_sync(0xffffffffu, (int)fixed, src), nfk = __shfl_sync(0xffffffffu, fk, src);
+    uint32_t nkeep = __shfl_sync(0xffffffffu, keep, src);
+    unsigned long long nstride = __shfl_sync(0xffffffffu, mystride, src);
+    if (node < 0) { ne = -1; nK = 1; no0 = 0; nfix = 0; nfk = 0; nkeep = 1u; nstride = 0; }
     bool pad = node < 0 || (node == 0 && k >= K0r);
     int korig = 0;   // the original option index behind slot digit k (kept options only; the pinned one for a fixed node)
     if (nfix) korig = nfk;
