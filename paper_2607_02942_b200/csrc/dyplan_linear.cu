@@ -320,8 +320,10 @@ __global__ void __launch_bounds__(128, (LT <= 4 ? 4 : 3)) k_lscore(const __grid_
     if (lane == 0) item = atomicAdd(&a.counter[0], 1u);
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= total) break;
-    const long long r = item / a.chunks;
-    const uint32_t c = item % a.chunks;
+    // items are handed out chunk by chunk across the requests, not request by request: a request's items are then
+    // spread over the whole launch and start from the J its earlier items published instead of all climbing at once
+    const long long r = item % (uint32_t)a.in.R;
+    const uint32_t c = item / (uint32_t)a.in.R;
     if (r != cur_req) {
       const uint32_t* blob = a.blob + (size_t)r * kLinBlobWords;
       __syncwarp();
