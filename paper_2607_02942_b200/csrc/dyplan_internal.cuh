@@ -113,7 +113,8 @@ struct CallState {
   // handed out is item (t * perm_sA) mod perm_nA among the first perm_nA (the regular items), then the same with perm_sB
   // among the rest (the small items of the tail); the strides are coprime to the counts and a little above the items of
   // one request, so consecutive hand-outs fall on consecutive requests and every request is visited all along the launch
-  uint32_t perm_nA, perm_sA, perm_sB, pad2;
+  uint32_t perm_nA, perm_sA, perm_sB;
+  uint32_t perm_sW;                 // wide class: the t-th item handed out is item (t * perm_sW) mod total_items
 };
 // outer indices per item of request r before rounding (k_plan and k_fscore must agree)
 __host__ __device__ inline unsigned long long fast_pif_of(unsigned long long pif, uint32_t tail_start, long long r) {

@@ -282,7 +282,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) k_score(const CallArgs a) 
 
   for (;;) {
     if (tid == 0) {
-      const uint32_t it = atomicAdd(&a.st->next_item, 1u);
+      uint32_t it = atomicAdd(&a.st->next_item, 1u);
+      // hand-out order: strided across the requests (CallState.perm_sW), so that a request's items do not all start at once
+      if (it < total_items) it = (uint32_t)(((unsigned long long)it * a.st->perm_sW) % total_items);
       s_item = it;
       if (it < total_items) {
         // largest r with item_off[r] <= it

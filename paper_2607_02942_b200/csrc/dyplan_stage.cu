@@ -581,7 +581,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
         st->slow_steps = 0; st->bound_skipped = 0;
         st->total_items = 0; st->next_item = 0; st->total_items_f = 0; st->next_item_f = 0;
         st->fast_requests = 0; st->small_call_f = 1u; st->tail_start_f = 0xffffffffu; st->approx_requests = 0; st->small_requests = is_small; st->pad0 = 0;
-        st->perm_nA = 0; st->perm_sA = 1; st->perm_sB = 1; st->pad2 = 0;
+        st->perm_nA = 0; st->perm_sA = 1; st->perm_sB = 1; st->perm_sW = 1;
       }
       return;
     }
@@ -702,7 +702,7 @@ __global__ void __launch_bounds__(1024) k_plan(CallArgs a) {
       st->perm_nA = nA;
       st->perm_sA = stride_for(nA, (nA + reqs - 1) / reqs);
       st->perm_sB = stride_for(nB, (uint32_t)((4ull * nB + reqs - 1) / reqs));   // (a sixteenth of the requests, 4x the items each: roughly)
-      st->pad2 = 0;
+      st->perm_sW = stride_for(total_items_w, (uint32_t)((total_items_w + (unsigned long long)R - 1) / (unsigned long long)R));
     }
     st->total_outer = total_w + total_f; st->total_plans = total_plans; st->per_item_outer = pio; st->per_item_outer_f = pif;
     st->slow_steps = 0; st->bound_skipped = 0;
